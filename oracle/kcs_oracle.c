@@ -1,0 +1,666 @@
+/*
+ * kcs_oracle.c -- ORACLE (test infrastructure, NOT the product).  See kcs_oracle.h.
+ *
+ * Plain fp64 C.  Every function cites the passage it follows:
+ *   P:<n>  = /root/reference/PAPER.md line n        BJ = /root/repo/BASELINE.json
+ *   S8c-X  = SURVEY.md section 8(c), reading X (frozen choices; repeated in DESIGN.md)
+ * No blocking, fusion or reordering beyond what the definitions state; OpenMP only
+ * distributes independent outer iterations (frames, slices, voxels).
+ */
+#define _GNU_SOURCE
+#include "kcs_oracle.h"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int kcso_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Geometry.  S8c-P1, P2 (Q1, Q3, Q4): voxel centres X_i = (i-(nx-1)/2) vx, angle theta_a = pi a/A,
+ * bin centre s_b = (b-(B-1)/2) bin_mm, step u_k = (k-(K-1)/2) step_mm,
+ * sample (X,Y) = (s cos - u sin, s sin + u cos), continuous index fx = X/vx + (nx-1)/2.
+ * ------------------------------------------------------------------------------------------ */
+static void angle_cos_sin(const kcso_config *c, int a, double *cs, double *sn) {
+    const double th = M_PI * (double)a / (double)c->n_angles;
+    *cs = cos(th);
+    *sn = sin(th);
+}
+static void sample_index(const kcso_config *c, double cs, double sn, int b, int k, double *fx, double *fy) {
+    const double s = ((double)b - 0.5 * (double)(c->n_bins - 1)) * c->bin_mm;
+    const double u = ((double)k - 0.5 * (double)(c->n_steps - 1)) * c->step_mm;
+    const double X = s * cs - u * sn;
+    const double Y = s * sn + u * cs;
+    *fx = X / c->vx + 0.5 * (double)(c->nx - 1);
+    *fy = Y / c->vy + 0.5 * (double)(c->ny - 1);
+}
+
+static int subset_count(const kcso_config *c, int subset) {
+    return subset < 0 ? c->n_angles : c->n_angles / c->n_subsets;
+}
+/* S8c-P5 (Q5): subset s = {a : a mod S == s}; the la-th angle of subset s is a = s + la*S. */
+static int subset_angle(const kcso_config *c, int subset, int la) {
+    return subset < 0 ? la : subset + la * c->n_subsets;
+}
+
+/* Q2: mask = {X^2+Y^2 <= ((min(nx,ny,B,K)/2 - 1) vx)^2}, same for every z. */
+void kcso_default_mask(const kcso_config *c, unsigned char *m) {
+    int mn = c->nx;
+    if (c->ny < mn) mn = c->ny;
+    if (c->n_bins < mn) mn = c->n_bins;
+    if (c->n_steps < mn) mn = c->n_steps;
+    const double rad = (0.5 * (double)mn - 1.0) * c->vx;
+    for (int j = 0; j < c->ny; ++j)
+        for (int i = 0; i < c->nx; ++i) {
+            const double X = ((double)i - 0.5 * (double)(c->nx - 1)) * c->vx;
+            const double Y = ((double)j - 0.5 * (double)(c->ny - 1)) * c->vy;
+            m[(size_t)j * c->nx + i] = (X * X + Y * Y <= rad * rad) ? 1 : 0;
+        }
+}
+
+static const unsigned char *get_mask(const kcso_config *c, unsigned char **owned) {
+    *owned = NULL;
+    if (c->mask) return c->mask;
+    *owned = (unsigned char *)malloc((size_t)c->nx * c->ny);
+    kcso_default_mask(c, *owned);
+    return *owned;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Projector.  S8c-P2, P3: value = bilinear interpolation on the 2x2 pixels around the sample,
+ * pixels outside the image contribute 0; (A f)[z,a,b] = step_mm * sum_k value.  Slices are
+ * independent 2-D problems (BJ configs[2],[3] "direct-plane sinograms").  P:64-67 (p_vd).
+ * ------------------------------------------------------------------------------------------ */
+static double pix(const double *img, int nx, int ny, int i, int j) {
+    return (i >= 0 && i < nx && j >= 0 && j < ny) ? img[(size_t)j * nx + i] : 0.0;
+}
+
+void kcso_forward_project(const kcso_config *c, const double *x, double *y, int subset, int nf) {
+    const int As = subset_count(c, subset);
+    const size_t V2 = (size_t)c->nx * c->ny;
+    const size_t R2 = (size_t)As * c->n_bins;
+    const long nimg = (long)nf * c->nz;
+#pragma omp parallel for schedule(dynamic, 1) collapse(2)
+    for (long tz = 0; tz < nimg; ++tz) {
+        for (int la = 0; la < As; ++la) {
+            const double *img = x + (size_t)tz * V2;
+            double *sino = y + (size_t)tz * R2;
+            const int a = subset_angle(c, subset, la);
+            double cs, sn;
+            angle_cos_sin(c, a, &cs, &sn);
+            for (int b = 0; b < c->n_bins; ++b) {
+                double acc = 0.0;
+                for (int k = 0; k < c->n_steps; ++k) {
+                    double fx, fy;
+                    sample_index(c, cs, sn, b, k, &fx, &fy);
+                    const int i0 = (int)floor(fx), j0 = (int)floor(fy);
+                    const double wx = fx - (double)i0, wy = fy - (double)j0;
+                    acc += (1.0 - wx) * (1.0 - wy) * pix(img, c->nx, c->ny, i0, j0) +
+                           wx * (1.0 - wy) * pix(img, c->nx, c->ny, i0 + 1, j0) +
+                           (1.0 - wx) * wy * pix(img, c->nx, c->ny, i0, j0 + 1) +
+                           wx * wy * pix(img, c->nx, c->ny, i0 + 1, j0 + 1);
+                }
+                sino[(size_t)la * c->n_bins + b] = c->step_mm * acc;
+            }
+        }
+    }
+}
+
+/* S8c-P4: A^T is the exact matrix transpose, implemented as the scatter of the loop above. */
+static void back_project_slice(const kcso_config *c, const double *sino, double *img, int subset) {
+    const int As = subset_count(c, subset);
+    const size_t V2 = (size_t)c->nx * c->ny;
+    memset(img, 0, V2 * sizeof(double));
+    for (int la = 0; la < As; ++la) {
+        const int a = subset_angle(c, subset, la);
+        double cs, sn;
+        angle_cos_sin(c, a, &cs, &sn);
+        for (int b = 0; b < c->n_bins; ++b) {
+            const double g = c->step_mm * (sino ? sino[(size_t)la * c->n_bins + b] : 1.0);
+            for (int k = 0; k < c->n_steps; ++k) {
+                double fx, fy;
+                sample_index(c, cs, sn, b, k, &fx, &fy);
+                const int i0 = (int)floor(fx), j0 = (int)floor(fy);
+                const double wx = fx - (double)i0, wy = fy - (double)j0;
+                const double w[4] = {(1.0 - wx) * (1.0 - wy), wx * (1.0 - wy), (1.0 - wx) * wy, wx * wy};
+                const int ii[4] = {i0, i0 + 1, i0, i0 + 1};
+                const int jj[4] = {j0, j0, j0 + 1, j0 + 1};
+                for (int q = 0; q < 4; ++q)
+                    if (ii[q] >= 0 && ii[q] < c->nx && jj[q] >= 0 && jj[q] < c->ny)
+                        img[(size_t)jj[q] * c->nx + ii[q]] += w[q] * g;
+            }
+        }
+    }
+}
+
+void kcso_back_project(const kcso_config *c, const double *q, double *b, int subset, int nf) {
+    const int As = subset_count(c, subset);
+    const size_t V2 = (size_t)c->nx * c->ny;
+    const size_t R2 = (size_t)As * c->n_bins;
+    const long nimg = (long)nf * c->nz;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long tz = 0; tz < nimg; ++tz)
+        back_project_slice(c, q + (size_t)tz * R2, b + (size_t)tz * V2, subset);
+}
+
+void kcso_sensitivity(const kcso_config *c, int subset, double *sens) {
+    back_project_slice(c, NULL, sens, subset);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * OSL update.  P:62-75 eq. 2-3 with the readings S8c-O2, Q7 (sign: prior pulls x toward F),
+ * Q8 (Poisson-matched sigma^2 = max(F,eps)/S), Q9 (D >= 0.1 S), Q10 (zero sensitivity -> 0), Q2 (mask).
+ *   D = S (1 + beta (x - F)/max(F,1e-20))      [KCSO_PRIOR_POISSON_MATCHED]
+ *   D = S + beta (x - F)/sigma2                [KCSO_PRIOR_ABSOLUTE]
+ *   x <- x * bp / max(D, 0.1 S);  x <- 0 where S <= 1e-12 max(S) or outside the mask.
+ * ------------------------------------------------------------------------------------------ */
+void kcso_osl_update(const kcso_config *c, double *x, const double *bp, const double *sens,
+                     const double *F, double beta, int prior_mode, double sigma2, int nf) {
+    unsigned char *owned;
+    const unsigned char *mask = get_mask(c, &owned);
+    const size_t V2 = (size_t)c->nx * c->ny;
+    double smax = 0.0;
+    for (size_t p = 0; p < V2; ++p)
+        if (sens[p] > smax) smax = sens[p];
+    const long nimg = (long)nf * c->nz;
+#pragma omp parallel for schedule(static)
+    for (long tz = 0; tz < nimg; ++tz) {
+        for (size_t p = 0; p < V2; ++p) {
+            const size_t idx = (size_t)tz * V2 + p;
+            const double S = sens[p];
+            if (!mask[p] || S <= 1e-12 * smax) {
+                x[idx] = 0.0;
+                continue;
+            }
+            double D;
+            if (prior_mode == KCSO_PRIOR_POISSON_MATCHED)
+                D = S * (1.0 + beta * (x[idx] - F[idx]) / fmax(F[idx], 1e-20));
+            else
+                D = S + beta * (x[idx] - F[idx]) / sigma2;
+            D = fmax(D, 0.1 * S);
+            x[idx] = x[idx] * bp[idx] / D;
+        }
+    }
+    free(owned);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Kinetic model.  BJ configs[0] (1)-(3); S8c-K1..K6.  Times in minutes.
+ *   Cp(t) = sum_i (alpha_i + beta_i t) e^{-lambda_i t},
+ *           (alpha,beta) = (-A2-A3, A1), (A2,0), (A3,0)                                  [K1]
+ *   a = k2+k3, B1 = K1 k2/a, B2 = K1 k3/a
+ *   Ct = vB Cp + (1-vB) [B1 (e^{-a.} conv Cp) + B2 (1 conv Cp)]                          [K2]
+ *   F_m = int_{ts_m}^{te_m} Ct dt  (integral, not average; Q11)                          [K3]
+ * Building block: P_n(r;t) = int_0^t u^n e^{-r u} du.
+ * ------------------------------------------------------------------------------------------ */
+static double Pn(int n, double r, double t) {
+    /* P_n(r;t) = t^{n+1} e^{-rt} sum_{j>=0} (rt)^j n!/(n+1+j)!   (all terms positive, r >= 0);
+     * for r < 0 the plain power series t^{n+1} sum_k (-rt)^k/(k!(n+k+1)) has positive terms. */
+    if (t <= 0.0) return 0.0;
+    const double xr = r * t;
+    double tp = t;
+    for (int q = 0; q < n; ++q) tp *= t; /* t^{n+1} */
+    if (n == 0) return (r == 0.0) ? t : -expm1(-xr) / r;
+    if (n == 1 && xr >= 1.0) return (1.0 - exp(-xr) * (1.0 + xr)) / (r * r); /* closed form, no cancellation here */
+    if (r >= 0.0) {
+        double term = 1.0 / (double)(n + 1), sum = term;
+        for (int j = 0; j < 2000; ++j) {
+            term *= xr / (double)(n + 2 + j);
+            sum += term;
+            if (term < 1e-18 * sum && (double)j > xr) break;
+        }
+        return tp * exp(-xr) * sum;
+    } else {
+        double term = 1.0, sum = 1.0 / (double)(n + 1);
+        for (int k = 1; k < 2000; ++k) {
+            term *= -xr / (double)k;
+            const double add = term / (double)(n + k + 1);
+            sum += add;
+            if (add < 1e-18 * sum && (double)k > -xr) break;
+        }
+        return tp * sum;
+    }
+}
+
+static void feng_ab(const kcso_config *c, double al[3], double be[3]) {
+    al[0] = -c->feng_A[1] - c->feng_A[2];
+    be[0] = c->feng_A[0];
+    al[1] = c->feng_A[1];
+    be[1] = 0.0;
+    al[2] = c->feng_A[2];
+    be[2] = 0.0;
+}
+
+static double Cp_at(const kcso_config *c, double t) {
+    double al[3], be[3], s = 0.0;
+    feng_ab(c, al, be);
+    for (int i = 0; i < 3; ++i) s += (al[i] + be[i] * t) * exp(-c->feng_lambda[i] * t);
+    return s;
+}
+
+void kcso_input_function(const kcso_config *c, const double *t, int n, double *cp) {
+    for (int q = 0; q < n; ++q) cp[q] = Cp_at(c, t[q]);
+}
+
+/* K4: ICp(t) = sum_i alpha_i P0(lambda_i;t) + beta_i P1(lambda_i;t). */
+double kcso_ICp(const kcso_config *c, double t) {
+    double al[3], be[3], s = 0.0;
+    feng_ab(c, al, be);
+    for (int i = 0; i < 3; ++i) s += al[i] * Pn(0, c->feng_lambda[i], t) + be[i] * Pn(1, c->feng_lambda[i], t);
+    return s;
+}
+
+/* K4: R_a(t) = (e^{-a.} conv Cp)(t)
+ *   = sum_i alpha_i E_i + beta_i [t e^{-lambda_i t} - E_i]/c_i,  c_i = a - lambda_i,
+ *   E_i = (e^{-lambda_i t} - e^{-a t})/c_i = e^{-lambda_i t} P0(c_i; t)   (stable for every c_i),
+ *   [t e^{-lambda t} - E]/c = e^{-lambda t} (t - P0(c;t))/c = e^{-lambda t} P1'(c;t),
+ *   with (t - P0(c;t))/c = int_0^t (1-e^{-cu})/c du = int_0^t P0(c;u) du, evaluated as
+ *   t^2 sum_n (-ct)^n/(n+2)! for |ct| < 0.5 and directly otherwise. */
+static double P0int_over(double cc, double t) { /* (t - P0(c;t))/c */
+    const double z = cc * t;
+    if (fabs(z) < 0.5) {
+        double term = 0.5, sum = 0.5; /* n = 0: 1/2! */
+        for (int n = 1; n < 40; ++n) {
+            term *= -z / (double)(n + 2);
+            sum += term;
+        }
+        return t * t * sum;
+    }
+    return (t - Pn(0, cc, t)) / cc;
+}
+
+double kcso_R(const kcso_config *c, double a, double t) {
+    double al[3], be[3], s = 0.0;
+    feng_ab(c, al, be);
+    for (int i = 0; i < 3; ++i) {
+        const double li = c->feng_lambda[i], ci = a - li, el = exp(-li * t);
+        s += al[i] * el * Pn(0, ci, t);
+        if (be[i] != 0.0) s += be[i] * el * P0int_over(ci, t);
+    }
+    return s;
+}
+
+/* K4: G_a(t) = int_0^t R_a = sum_i alpha_i D_i + beta_i T_i with, for f(r) = P0(r;t)
+ * (so f^(n)(r) = (-1)^n P_n(r;t)) and c = a - lambda_i:
+ *   D_i = (P0(lambda_i;t) - P0(a;t))/c           = -(f(a)-f(lambda))/c
+ *   T_i = P1(lambda_i;t)/c - D_i/c               = (f(a)-f(lambda)-f'(lambda) c)/c^2
+ * and their a-derivatives dD = (P1(a;t) - D)/c, dT = -(dD + T)/c.
+ * For |c| <= 0.05 the same four quantities are summed from the Taylor series of f about lambda
+ * (removable singularity; K5 "repeated node = derivative"):
+ *   D = -sum_{n>=1} f^(n) c^{n-1}/n!,  T = sum_{n>=2} f^(n) c^{n-2}/n!,
+ *   dD = -sum_{n>=2} (n-1) f^(n) c^{n-2}/n!,  dT = sum_{n>=3} (n-2) f^(n) c^{n-3}/n!. */
+static void DT_terms(double lam, double a, double t, int double_pole, double *D, double *T, double *dD, double *dT) {
+    const double cc = a - lam;
+    (void)double_pole;
+    if (fabs(cc) > 0.05) {
+        const double P0l = Pn(0, lam, t), P0a = Pn(0, a, t), P1l = Pn(1, lam, t), P1a = Pn(1, a, t);
+        *D = (P0l - P0a) / cc;
+        *T = (P1l - *D) / cc;
+        *dD = (P1a - *D) / cc;
+        *dT = -(*dD + *T) / cc;
+        return;
+    }
+    /* P_n(lambda;t), n = 0..NT, by the integration-by-parts identity P_{n-1} = (r P_n + t^n e^{-rt})/n run
+     * downwards from P_NT (series); downwards is the stable direction. */
+    enum { NT = 48 };
+    double P[NT + 1], tpow[NT + 1];
+    tpow[0] = 1.0;
+    for (int n = 1; n <= NT; ++n) tpow[n] = tpow[n - 1] * t;
+    P[NT] = Pn(NT, lam, t);
+    const double elt = exp(-lam * t);
+    for (int n = NT; n >= 1; --n) P[n - 1] = (lam * P[n] + tpow[n] * elt) / (double)n;
+    double d = 0.0, tt = 0.0, dd = 0.0, dt = 0.0;
+    double fact = 1.0;             /* n! */
+    double cp[NT + 1];             /* c^k */
+    cp[0] = 1.0;
+    for (int n = 1; n <= NT; ++n) cp[n] = cp[n - 1] * cc;
+    for (int n = 1; n <= NT; ++n) {
+        fact *= (double)n;
+        const double fn = ((n & 1) ? -1.0 : 1.0) * P[n]; /* f^(n)(lambda) */
+        d += -fn * cp[n - 1] / fact;
+        if (n >= 2) {
+            tt += fn * cp[n - 2] / fact;
+            dd += -(double)(n - 1) * fn * cp[n - 2] / fact;
+        }
+        if (n >= 3) dt += (double)(n - 2) * fn * cp[n - 3] / fact;
+    }
+    *D = d;
+    *T = tt;
+    *dD = dd;
+    *dT = dt;
+}
+
+double kcso_G(const kcso_config *c, double a, double t) {
+    double al[3], be[3], s = 0.0;
+    feng_ab(c, al, be);
+    for (int i = 0; i < 3; ++i) {
+        double D, T, dD, dT;
+        DT_terms(c->feng_lambda[i], a, t, be[i] != 0.0, &D, &T, &dD, &dT);
+        s += al[i] * D + be[i] * T;
+    }
+    return s;
+}
+
+double kcso_dGda(const kcso_config *c, double a, double t) {
+    double al[3], be[3], s = 0.0;
+    feng_ab(c, al, be);
+    for (int i = 0; i < 3; ++i) {
+        double D, T, dD, dT;
+        DT_terms(c->feng_lambda[i], a, t, be[i] != 0.0, &D, &T, &dD, &dT);
+        s += al[i] * dD + be[i] * dT;
+    }
+    return s;
+}
+
+/* K2: instantaneous tissue curve (used by the quadrature pins only). */
+double kcso_Ct(const kcso_config *c, const double xi[4], double t) {
+    const double K1 = xi[0], k2 = xi[1], k3 = xi[2], vB = xi[3], a = k2 + k3;
+    double tissue;
+    if (a > 0.0)
+        tissue = K1 * k2 / a * kcso_R(c, a, t) + K1 * k3 / a * kcso_ICp(c, t);
+    else
+        tissue = K1 * kcso_ICp(c, t);
+    return vB * Cp_at(c, t) + (1.0 - vB) * tissue;
+}
+
+/* K3, K6 for one voxel: F_m and (optionally) the four partial derivatives.
+ *   F_m     = vB dICp_m + (1-vB) [B1 W_m(a) + B2 W_m(0)],  W_m(a) = G_a(te) - G_a(ts)
+ *   dF/dK1  = (1-vB) [(k2/a) W(a) + (k3/a) W(0)]
+ *   dF/dk2  = (1-vB) [(K1 k3/a^2)(W(a)-W(0)) + B1 W'(a)]
+ *   dF/dk3  = (1-vB) [(K1 k2/a^2)(W(0)-W(a)) + B1 W'(a)]
+ *   dF/dvB  = dICp - [B1 W(a) + B2 W(0)]                                   (P:85-89 analytic) */
+/* The two voxel-independent tables dICp_m and W_m(0) are computed once per call (memoisation only). */
+static double *frame_tables(const kcso_config *c) {
+    const int T = c->n_frames;
+    double *tab = (double *)malloc(sizeof(double) * 2 * T);
+    for (int m = 0; m < T; ++m) {
+        const double ts = c->t_start_min[m], te = c->t_end_min[m];
+        tab[m] = kcso_ICp(c, te) - kcso_ICp(c, ts);
+        tab[T + m] = kcso_G(c, 0.0, te) - kcso_G(c, 0.0, ts);
+    }
+    return tab;
+}
+
+static void tac_voxel(const kcso_config *c, const double *tab, const double xi[4], double *F,
+                      double *J /* [4][T] or NULL */) {
+    const int T = c->n_frames;
+    const double K1 = xi[0], k2 = xi[1], k3 = xi[2], vB = xi[3], a = k2 + k3;
+    for (int m = 0; m < T; ++m) {
+        const double ts = c->t_start_min[m], te = c->t_end_min[m];
+        const double dICp = tab[m];
+        const double W0 = tab[T + m];
+        if (a > 0.0) {
+            const double Wa = kcso_G(c, a, te) - kcso_G(c, a, ts);
+            const double B1 = K1 * k2 / a, B2 = K1 * k3 / a;
+            F[m] = vB * dICp + (1.0 - vB) * (B1 * Wa + B2 * W0);
+            if (J) {
+                const double dWa = kcso_dGda(c, a, te) - kcso_dGda(c, a, ts);
+                J[0 * T + m] = (1.0 - vB) * ((k2 / a) * Wa + (k3 / a) * W0);
+                J[1 * T + m] = (1.0 - vB) * ((K1 * k3 / (a * a)) * (Wa - W0) + B1 * dWa);
+                J[2 * T + m] = (1.0 - vB) * ((K1 * k2 / (a * a)) * (W0 - Wa) + B1 * dWa);
+                J[3 * T + m] = dICp - (B1 * Wa + B2 * W0);
+            }
+        } else { /* k2 = k3 = 0: bracket of K2 reduces to K1 (1 conv Cp) */
+            F[m] = vB * dICp + (1.0 - vB) * K1 * W0;
+            if (J) {
+                J[0 * T + m] = (1.0 - vB) * W0;
+                J[1 * T + m] = 0.0;
+                J[2 * T + m] = 0.0;
+                J[3 * T + m] = dICp - K1 * W0;
+            }
+        }
+    }
+}
+
+void kcso_kinetic_eval(const kcso_config *c, const double *theta, double *F, double *J, long V) {
+    const int T = c->n_frames;
+    double *tab = frame_tables(c);
+#pragma omp parallel
+    {
+        double *Fv = (double *)malloc(sizeof(double) * T);
+        double *Jv = (double *)malloc(sizeof(double) * 4 * T);
+#pragma omp for schedule(dynamic, 64)
+        for (long v = 0; v < V; ++v) {
+            const double xi[4] = {theta[0 * V + v], theta[1 * V + v], theta[2 * V + v], theta[3 * V + v]};
+            tac_voxel(c, tab, xi, Fv, J ? Jv : NULL);
+            for (int m = 0; m < T; ++m) {
+                F[(size_t)m * V + v] = Fv[m];
+                if (J)
+                    for (int p = 0; p < 4; ++p) J[((size_t)p * T + m) * V + v] = Jv[p * T + m];
+            }
+        }
+        free(Fv);
+        free(Jv);
+    }
+    free(tab);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * MAP-LM.  P:91-114 eq. 4-7 with the readings S8c-L1..L3, Q12 (standard Huber), Q13 (6-neighbourhood,
+ * free boundary, in-mask neighbours only), Q14 (gamma as passed), Q15 (lambda rule), Q16 (box).
+ * ------------------------------------------------------------------------------------------ */
+static double huber(double t, double delta) { /* eq. 5 with Q12: t^2/2 | delta|t| - delta^2/2 */
+    const double at = fabs(t);
+    return at <= delta ? 0.5 * t * t : delta * at - 0.5 * delta * delta;
+}
+static double huber_d(double t, double delta) { /* eq. 6 with Q12: clamp(t,-delta,delta) */
+    return t < -delta ? -delta : (t > delta ? delta : t);
+}
+
+static const double BOX_LO[4] = {0.0, 1e-4, 0.0, 0.0};
+static const double BOX_HI[4] = {2.0, 2.0, 1.0, 1.0};
+
+static double objective(const kcso_config *c, const double *xv, const double xi[4], const double *Fv,
+                        const double *nbr, int n_nbr, double gamma, double delta) {
+    const int T = c->n_frames;
+    double phi = 0.0;
+    for (int m = 0; m < T; ++m) phi += 0.5 * (xv[m] - Fv[m]) * (xv[m] - Fv[m]);
+    for (int p = 0; p < 4; ++p)
+        for (int q = 0; q < n_nbr; ++q) phi += gamma * huber(xi[p] - nbr[q * 4 + p], delta);
+    return phi;
+}
+
+double kcso_lm_objective(const kcso_config *c, const double *xv, const double xi[4],
+                         const double *nbr, int n_nbr, double gamma, double delta) {
+    double *Fv = (double *)malloc(sizeof(double) * c->n_frames);
+    double *tab = frame_tables(c);
+    tac_voxel(c, tab, xi, Fv, NULL);
+    const double phi = objective(c, xv, xi, Fv, nbr, n_nbr, gamma, delta);
+    free(Fv);
+    free(tab);
+    return phi;
+}
+
+/* 4x4 Cholesky solve of M d = g; returns 0 when a pivot is not positive. */
+static int chol4_solve(const double M[4][4], const double g[4], double d[4]) {
+    double L[4][4] = {{0}};
+    for (int i = 0; i < 4; ++i)
+        for (int j = 0; j <= i; ++j) {
+            double s = M[i][j];
+            for (int k = 0; k < j; ++k) s -= L[i][k] * L[j][k];
+            if (i == j) {
+                if (!(s > 0.0) || !isfinite(s)) return 0;
+                L[i][i] = sqrt(s);
+            } else
+                L[i][j] = s / L[j][j];
+        }
+    double z[4];
+    for (int i = 0; i < 4; ++i) {
+        double s = g[i];
+        for (int k = 0; k < i; ++k) s -= L[i][k] * z[k];
+        z[i] = s / L[i][i];
+    }
+    for (int i = 3; i >= 0; --i) {
+        double s = z[i];
+        for (int k = i + 1; k < 4; ++k) s -= L[k][i] * d[k];
+        d[i] = s / L[i][i];
+    }
+    return 1;
+}
+
+/* One LM step for one voxel (L2). xi in/out, lam in/out; returns Phi after the step. */
+static double lm_step_voxel(const kcso_config *c, const double *tab, const double *xv, double xi[4], double *lam,
+                            const double *nbr, int n_nbr, double gamma, double delta,
+                            double *Fv, double *Jv, double *Ft) {
+    const int T = c->n_frames;
+    tac_voxel(c, tab, xi, Fv, Jv);
+    const double phi_old = objective(c, xv, xi, Fv, nbr, n_nbr, gamma, delta);
+    double JtJ[4][4] = {{0}}, g[4] = {0};
+    for (int p = 0; p < 4; ++p) {
+        for (int q = 0; q < 4; ++q)
+            for (int m = 0; m < T; ++m) JtJ[p][q] += Jv[p * T + m] * Jv[q * T + m];
+        for (int m = 0; m < T; ++m) g[p] += Jv[p * T + m] * (xv[m] - Fv[m]);
+        for (int q = 0; q < n_nbr; ++q) g[p] -= gamma * huber_d(xi[p] - nbr[q * 4 + p], delta);
+    }
+    if (!(*lam > 0.0)) { /* Q15: first use */
+        double mx = 0.0;
+        for (int p = 0; p < 4; ++p)
+            if (JtJ[p][p] > mx) mx = JtJ[p][p];
+        *lam = 1e-3 * mx;
+    }
+    double M[4][4], d[4];
+    for (int p = 0; p < 4; ++p)
+        for (int q = 0; q < 4; ++q) M[p][q] = JtJ[p][q] + (p == q ? *lam : 0.0);
+    if (!chol4_solve(M, g, d)) { /* not positive definite: treated as a rejected step */
+        *lam = fmin(10.0 * *lam, 1e30);
+        return phi_old;
+    }
+    double xt[4];
+    for (int p = 0; p < 4; ++p) xt[p] = fmin(fmax(xi[p] + d[p], BOX_LO[p]), BOX_HI[p]);
+    tac_voxel(c, tab, xt, Ft, NULL);
+    const double phi_new = objective(c, xv, xt, Ft, nbr, n_nbr, gamma, delta);
+    if (phi_new <= phi_old) {
+        for (int p = 0; p < 4; ++p) xi[p] = xt[p];
+        *lam = fmax(*lam / 10.0, 1e-30);
+        return phi_new;
+    }
+    *lam = fmin(10.0 * *lam, 1e30);
+    return phi_old;
+}
+
+void kcso_map_lm(const kcso_config *c, const double *x, double *theta, double *lambda,
+                 double gamma, double delta, int n_steps, double *cost) {
+    unsigned char *owned;
+    const unsigned char *mask = get_mask(c, &owned);
+    const int T = c->n_frames, nx = c->nx, ny = c->ny, nz = c->nz;
+    const long V2 = (long)nx * ny, V = V2 * nz;
+    double *prev = (double *)malloc(sizeof(double) * 4 * V);
+    double *tab = frame_tables(c);
+    for (int step = 0; step < n_steps; ++step) {
+        memcpy(prev, theta, sizeof(double) * 4 * V); /* Jacobi: all voxels read the state at step start */
+#pragma omp parallel
+        {
+            double *xv = (double *)malloc(sizeof(double) * T);
+            double *Fv = (double *)malloc(sizeof(double) * T);
+            double *Ft = (double *)malloc(sizeof(double) * T);
+            double *Jv = (double *)malloc(sizeof(double) * 4 * T);
+#pragma omp for schedule(dynamic, 64)
+            for (long v = 0; v < V; ++v) {
+                const int z = (int)(v / V2), j = (int)((v % V2) / nx), i = (int)(v % nx);
+                if (!mask[(size_t)j * nx + i]) {
+                    if (cost) cost[v] = 0.0;
+                    continue;
+                }
+                double nbr[6 * 4];
+                int n_nbr = 0;
+                const int di[6] = {-1, 1, 0, 0, 0, 0}, dj[6] = {0, 0, -1, 1, 0, 0}, dz[6] = {0, 0, 0, 0, -1, 1};
+                for (int q = 0; q < 6; ++q) {
+                    const int ii = i + di[q], jj = j + dj[q], zz = z + dz[q];
+                    if (ii < 0 || ii >= nx || jj < 0 || jj >= ny || zz < 0 || zz >= nz) continue;
+                    if (!mask[(size_t)jj * nx + ii]) continue;
+                    const long w = (long)zz * V2 + (long)jj * nx + ii;
+                    for (int p = 0; p < 4; ++p) nbr[n_nbr * 4 + p] = prev[(size_t)p * V + w];
+                    ++n_nbr;
+                }
+                double xi[4];
+                for (int p = 0; p < 4; ++p) xi[p] = prev[(size_t)p * V + v];
+                for (int m = 0; m < T; ++m) xv[m] = x[(size_t)m * V + v];
+                double lam = lambda[v];
+                const double phi = lm_step_voxel(c, tab, xv, xi, &lam, nbr, n_nbr, gamma, delta, Fv, Jv, Ft);
+                for (int p = 0; p < 4; ++p) theta[(size_t)p * V + v] = xi[p];
+                lambda[v] = lam;
+                if (cost) cost[v] = phi;
+            }
+            free(xv);
+            free(Fv);
+            free(Ft);
+            free(Jv);
+        }
+    }
+    free(prev);
+    free(tab);
+    free(owned);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * OS pass and ICM iteration.  S8c-O1, O2, I; eq. 2.
+ *   yhat = scale A_s x_t + r_t ; q = y/yhat where yhat > 1e-12 else 0 ; b = scale A_s^T q ; S_s = scale A_s^T 1
+ * ------------------------------------------------------------------------------------------ */
+void kcso_os_pass(const kcso_config *c, const double *y, const double *r, int r_mode, double scale,
+                  double *x, const double *F, double beta) {
+    const int T = c->n_frames, S = c->n_subsets, A = c->n_angles, B = c->n_bins, As = A / S;
+    const size_t V2 = (size_t)c->nx * c->ny, V = V2 * c->nz;
+    const size_t Rs = (size_t)c->nz * As * B; /* rays per frame in one subset */
+    double *yh = (double *)malloc(sizeof(double) * T * Rs);
+    double *bp = (double *)malloc(sizeof(double) * T * V);
+    double *sens = (double *)malloc(sizeof(double) * V2);
+    for (int s = 0; s < S; ++s) {
+        kcso_forward_project(c, x, yh, s, T);
+        for (int t = 0; t < T; ++t)
+            for (int z = 0; z < c->nz; ++z)
+                for (int la = 0; la < As; ++la)
+                    for (int b = 0; b < B; ++b) {
+                        const size_t is = (((size_t)t * c->nz + z) * As + la) * B + b;
+                        const int a = s + la * S;
+                        const size_t ifull = (((size_t)t * c->nz + z) * A + a) * B + b;
+                        const double rr = r_mode == 0 ? r[t] : r[ifull];
+                        const double yhat = scale * yh[is] + rr;
+                        yh[is] = yhat > 1e-12 ? y[ifull] / yhat : 0.0;
+                    }
+        kcso_back_project(c, yh, bp, s, T);
+        for (size_t q = 0; q < (size_t)T * V; ++q) bp[q] *= scale;
+        kcso_sensitivity(c, s, sens);
+        for (size_t p = 0; p < V2; ++p) sens[p] *= scale;
+        kcso_osl_update(c, x, bp, sens, F, beta, KCSO_PRIOR_POISSON_MATCHED, 1.0, T);
+    }
+    free(yh);
+    free(bp);
+    free(sens);
+}
+
+void kcso_icm_iteration(const kcso_config *c, const double *y, const double *r, int r_mode, double scale,
+                        double *x, double *theta, double *lambda,
+                        double beta, double gamma, double delta, int n_lm) {
+    const int T = c->n_frames;
+    const size_t V = (size_t)c->nx * c->ny * c->nz;
+    double *F = (double *)malloc(sizeof(double) * T * V);
+    kcso_kinetic_eval(c, theta, F, NULL, (long)V);   /* F <- K(theta^{n-1}), held fixed during the pass */
+    kcso_os_pass(c, y, r, r_mode, scale, x, F, beta); /* (a) P:124 */
+    kcso_map_lm(c, x, theta, lambda, gamma, delta, n_lm, NULL); /* (b) P:125 */
+    free(F);
+}
+
+double kcso_poisson_loglik(const kcso_config *c, const double *y, const double *r, int r_mode,
+                           double scale, const double *x) {
+    const int T = c->n_frames, A = c->n_angles, B = c->n_bins;
+    const size_t R = (size_t)c->nz * A * B;
+    double *yh = (double *)malloc(sizeof(double) * T * R);
+    kcso_forward_project(c, x, yh, -1, T);
+    double ll = 0.0;
+    for (int t = 0; t < T; ++t)
+        for (size_t d = 0; d < R; ++d) {
+            const size_t q = (size_t)t * R + d;
+            const double yhat = scale * yh[q] + (r_mode == 0 ? r[t] : r[q]);
+            if (yhat > 0.0) ll += y[q] * log(yhat) - yhat;
+        }
+    free(yh);
+    return ll;
+}
