@@ -1,0 +1,481 @@
+// kcs_api.cu -- the C ABI of include/kcs.h: argument checking, context set-up (geometry and kinetic tables in
+// fp64 on the host), and the sequencing of kernels for each entry point.  No compute happens on the host.
+#include <climits>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "kcs_internal.cuh"
+
+namespace {
+
+thread_local std::string g_create_err;
+
+int fail(kcs_ctx *c, int code, const std::string &msg) {
+    if (c) c->err = msg;
+    else g_create_err = msg;
+    return code;
+}
+
+// ---- host quadrature for the voxel-independent kinetic tables (K3, K4) -------------------------------
+// 8-point Gauss-Legendre on `panels` equal panels; every integrand here is entire, so this is exact to rounding.
+template <class F>
+long double gl8(F f, long double a, long double b, int panels) {
+    static const long double xs[4] = {0.1834346424956498049L, 0.5255324099163289858L, 0.7966664774136267396L,
+                                      0.9602898564975362317L};
+    static const long double ws[4] = {0.3626837833783619830L, 0.3137066458778872873L, 0.2223810344533744706L,
+                                      0.1012285362903762591L};
+    if (!(b > a)) return 0.0L;
+    const long double h = (b - a) / panels;
+    long double sum = 0.0L;
+    for (int p = 0; p < panels; ++p) {
+        const long double mid = a + (p + 0.5L) * h, half = 0.5L * h;
+        long double s = 0.0L;
+        for (int q = 0; q < 4; ++q) s += ws[q] * (f(mid - half * xs[q]) + f(mid + half * xs[q]));
+        sum += s * half;
+    }
+    return sum;
+}
+
+int panels_for(long double len) {
+    int p = (int)std::ceil((double)len * 16.0);
+    return p < 64 ? 64 : p;
+}
+
+struct Feng {
+    long double al[3], be[3], lam[3];
+    long double Cp(long double t) const {
+        long double s = 0.0L;
+        for (int i = 0; i < 3; ++i) s += (al[i] + be[i] * t) * expl(-lam[i] * t);
+        return s;
+    }
+};
+
+void fill_boundary(const Feng &fe, double t, KBoundary &b) {
+    b.t = t;
+    const int np = panels_for(t);
+    for (int i = 0; i < 3; ++i) {
+        const long double l = fe.lam[i];
+        b.P0[i] = (double)gl8([&](long double u) { return expl(-l * u); }, 0.0L, t, np);
+    }
+    {
+        const long double l = fe.lam[0];
+        b.P1_0 = (double)gl8([&](long double u) { return u * expl(-l * u); }, 0.0L, t, np);
+    }
+    for (int i = 1; i < 3; ++i) {
+        const long double l = fe.lam[i];
+        for (int n = 1; n <= 4; ++n)
+            b.Pn[i - 1][n - 1] = (double)gl8([&](long double u) { return powl(u, n) * expl(-l * u); }, 0.0L, t, np);
+    }
+}
+
+int check_cfg(const kcs_config *c, std::string &why) {
+    if (c->nx <= 0 || c->ny <= 0 || c->nz <= 0 || c->n_angles <= 0 || c->n_bins < 3 || c->n_steps <= 0 ||
+        c->n_subsets <= 0 || !(c->vx > 0) || !(c->vy > 0) || !(c->bin_mm > 0) || !(c->step_mm > 0)) {
+        why = "non-positive size (n_bins must be >= 3)";
+        return KCS_ERR_SHAPE;
+    }
+    if (c->n_angles % c->n_subsets != 0) {
+        why = "n_subsets does not divide n_angles";
+        return KCS_ERR_SUBSET;
+    }
+    if (c->n_frames <= 0 || c->n_frames > KCS_MAX_FRAMES) {
+        why = "n_frames must be in [1, KCS_MAX_FRAMES]";
+        return KCS_ERR_FRAMES;
+    }
+    if (!c->t_start_min || !c->t_end_min) {
+        why = "frame tables are NULL";
+        return KCS_ERR_NULL;
+    }
+    for (int m = 0; m < c->n_frames; ++m)
+        if (!(c->t_end_min[m] > c->t_start_min[m]) || c->t_start_min[m] < 0.0) {
+            why = "frame with t_end <= t_start or negative start";
+            return KCS_ERR_FRAMES;
+        }
+    for (int i = 0; i < 3; ++i)
+        if (!(c->feng_lambda[i] > 0.f)) {
+            why = "feng_lambda must be positive";
+            return KCS_ERR_SHAPE;
+        }
+    for (int a = 0; a < c->n_angles; ++a) {
+        const double th = M_PI * a / c->n_angles, cs = std::fabs(std::cos(th)), sn = std::fabs(std::sin(th));
+        if ((cs * c->vx + sn * c->vy) / c->bin_mm > 1.5 || (sn * c->vx + cs * c->vy) / c->step_mm > 1.5) {
+            why = "voxel too large for the bin/step size: a voxel would see more than 3x3 ray samples per angle";
+            return KCS_ERR_SHAPE;
+        }
+    }
+    return KCS_OK;
+}
+
+template <class T>
+cudaError_t dalloc(kcs_ctx *c, T **p, size_t n) {
+    cudaError_t e = cudaMalloc((void **)p, n * sizeof(T));
+    if (e == cudaSuccess) c->ws_bytes += (long long)(n * sizeof(T));
+    return e;
+}
+
+int ensure_border(kcs_ctx *c, int Tp) {
+    if (c->xi_border_tp != Tp) {
+        KCS_CUDA_OK(c, cudaMemsetAsync(c->xi, 0, c->n_pix_pad * (size_t)Tp * sizeof(float), c->stream));
+        c->xi_border_tp = Tp;
+    }
+    return KCS_OK;
+}
+
+int pack_image(kcs_ctx *c, const float *planar, int nf, float *inner, int Tp) {
+    const KGeom &g = c->g;
+    return kcs_launch_pack(c, planar, c->n_vox, nf, inner, Tp, (long long)g.nz * g.ny, g.nx, g.ny,
+                           (long long)g.nyp * g.nxp, g.nxp, g.nxp + 1);
+}
+int unpack_image(kcs_ctx *c, const float *inner, int Tp, float *planar, int nf) {
+    const KGeom &g = c->g;
+    return kcs_launch_unpack(c, inner, Tp, planar, c->n_vox, nf, (long long)g.nz * g.ny, g.nx, g.ny,
+                             (long long)g.nyp * g.nxp, g.nxp, g.nxp + 1);
+}
+int pack_sino(kcs_ctx *c, const float *planar, int nf, float *inner, int Tp, int As) {
+    const KGeom &g = c->g;
+    return kcs_launch_pack(c, planar, (size_t)g.nz * As * g.B, nf, inner, Tp, (long long)g.nz * As, g.B, INT_MAX, 0, g.B, 0);
+}
+int unpack_sino(kcs_ctx *c, const float *inner, int Tp, float *planar, int nf, int As) {
+    const KGeom &g = c->g;
+    return kcs_launch_unpack(c, inner, Tp, planar, (size_t)g.nz * As * g.B, nf, (long long)g.nz * As, g.B, INT_MAX, 0, g.B,
+                             0);
+}
+
+int check_subset_frames(kcs_ctx *c, int subset, int f0, int nf) {
+    if (subset < -1 || subset >= c->cfg.n_subsets) return fail(c, KCS_ERR_SHAPE, "subset out of range");
+    if (f0 < 0 || nf <= 0 || f0 + nf > c->cfg.n_frames) return fail(c, KCS_ERR_SHAPE, "frame range out of [0, n_frames)");
+    return KCS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *kcs_last_error(const kcs_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+long long kcs_workspace_bytes(const kcs_ctx *ctx) { return ctx ? ctx->ws_bytes : 0; }
+long long kcs_launch_count(const kcs_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int kcs_set_stream(kcs_ctx *ctx, void *stream) {
+    if (!ctx) return KCS_ERR_NULL;
+    ctx->stream = (cudaStream_t)stream;
+    return KCS_OK;
+}
+
+int kcs_get_mask(const kcs_ctx *ctx, unsigned char *out) {
+    if (!ctx || !out) return KCS_ERR_NULL;
+    std::memcpy(out, ctx->h_mask.data(), ctx->h_mask.size());
+    return KCS_OK;
+}
+
+int kcs_destroy(kcs_ctx *c) {
+    if (!c) return KCS_ERR_NULL;
+    cudaStreamSynchronize(c->stream);
+    void *ptrs[] = {c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->xi, c->Fi,
+                    c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
+    for (void *p : ptrs)
+        if (p) cudaFree(p);
+    delete c;
+    return KCS_OK;
+}
+
+int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
+    if (!out || !cfg) return fail(nullptr, KCS_ERR_NULL, "kcs_create: NULL argument");
+    *out = nullptr;
+    std::string why;
+    int rc = check_cfg(cfg, why);
+    if (rc != KCS_OK) return fail(nullptr, rc, "kcs_create: " + why);
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, KCS_ERR_CUDA, "kcs_create: no CUDA device (this library has no CPU fallback)");
+    }
+    kcs_ctx *c = new (std::nothrow) kcs_ctx();
+    if (!c) return fail(nullptr, KCS_ERR_ALLOC, "kcs_create: host allocation failed");
+    c->cfg = *cfg;
+    c->ts.assign(cfg->t_start_min, cfg->t_start_min + cfg->n_frames);
+    c->te.assign(cfg->t_end_min, cfg->t_end_min + cfg->n_frames);
+    c->cfg.t_start_min = c->ts.data();
+    c->cfg.t_end_min = c->te.data();
+    c->cfg.mask_host = nullptr;
+    c->stream = (cudaStream_t)stream;
+    c->launches = 0;
+    c->ws_bytes = 0;
+    c->xi_border_tp = 0;
+    c->d_fwd = c->d_bwd = nullptr; c->d_frames = nullptr; c->d_mask = nullptr;
+    c->d_sens = c->d_smax = c->d_tmp_smax = nullptr;
+    c->xi = c->Fi = c->qi = c->yi = c->ri = c->r_pad = c->theta2 = nullptr;
+    c->st_y = c->st_r = c->st_x = c->st_theta = c->st_lambda = nullptr;
+    c->st_r_elems = 0;
+
+    const int nx = cfg->nx, ny = cfg->ny, nz = cfg->nz, A = cfg->n_angles, B = cfg->n_bins, K = cfg->n_steps, T = cfg->n_frames;
+    KGeom &g = c->g;
+    g.nx = nx; g.ny = ny; g.nz = nz; g.nxp = nx + 2; g.nyp = ny + 2;
+    g.A = A; g.B = B; g.K = K; g.S = cfg->n_subsets;
+    g.step_mm = cfg->step_mm;
+    g.cx = 0.5 * (nx - 1); g.cy = 0.5 * (ny - 1); g.cb = 0.5 * (B - 1); g.ck = 0.5 * (K - 1);
+    c->n_vox = (size_t)nz * ny * nx;
+    c->n_pix_pad = (size_t)nz * g.nyp * g.nxp;
+    c->n_ray_all = (size_t)nz * A * B;
+
+    // P1: angle tables (fp64)
+    std::vector<double4> fw(A), bw(A);
+    for (int a = 0; a < A; ++a) {
+        const double th = M_PI * (double)a / (double)A, cs = std::cos(th), sn = std::sin(th);
+        const double vx = cfg->vx, vy = cfg->vy, bin = cfg->bin_mm, st = cfg->step_mm;
+        fw[a] = make_double4(bin * cs / vx, -st * sn / vx, bin * sn / vy, st * cs / vy);
+        bw[a] = make_double4(vx * cs / bin, vy * sn / bin, -vx * sn / st, vy * cs / st);
+    }
+    // Q2: field-of-view mask
+    c->h_mask.resize((size_t)nx * ny);
+    if (cfg->mask_host) {
+        for (size_t q = 0; q < c->h_mask.size(); ++q) c->h_mask[q] = cfg->mask_host[q] ? 1 : 0;
+    } else {
+        int mn = nx < ny ? nx : ny;
+        if (B < mn) mn = B;
+        if (K < mn) mn = K;
+        const double rad = (0.5 * mn - 1.0) * cfg->vx;
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const double X = (i - g.cx) * cfg->vx, Y = (j - g.cy) * cfg->vy;
+                c->h_mask[(size_t)j * nx + i] = (X * X + Y * Y <= rad * rad) ? 1 : 0;
+            }
+    }
+    // K1, K3, K4: kinetic tables (fp64 via long-double quadrature)
+    Feng fe;
+    fe.al[0] = -(long double)cfg->feng_A[1] - (long double)cfg->feng_A[2];
+    fe.be[0] = cfg->feng_A[0];
+    fe.al[1] = cfg->feng_A[1]; fe.be[1] = 0.0L;
+    fe.al[2] = cfg->feng_A[2]; fe.be[2] = 0.0L;
+    for (int i = 0; i < 3; ++i) fe.lam[i] = cfg->feng_lambda[i];
+    std::vector<KFrame> frames(T);
+    for (int m = 0; m < T; ++m) {
+        KFrame &f = frames[m];
+        const double ts = c->ts[m], te = c->te[m];
+        fill_boundary(fe, ts, f.b[0]);
+        fill_boundary(fe, te, f.b[1]);
+        f.dt = te - ts;
+        const long double ICp_ts = gl8([&](long double u) { return fe.Cp(u); }, 0.0L, ts, panels_for(ts));
+        const int np = panels_for(f.dt);
+        f.dICp = (double)gl8([&](long double u) { return fe.Cp(u); }, ts, te, np);
+        // W0 = int_ts^te ICp(t) dt = dt ICp(ts) + int_ts^te (te - u) Cp(u) du
+        f.W0 = (double)((long double)f.dt * ICp_ts +
+                        gl8([&](long double u) { return ((long double)te - u) * fe.Cp(u); }, ts, te, np));
+        f.contiguous = (m > 0 && c->ts[m] == c->te[m - 1]) ? 1 : 0;
+        if (m > 0 && std::fabs(f.dt - frames[m - 1].dt) <= 1e-12 * f.dt) {
+            f.dt = frames[m - 1].dt;  // same duration class: per-duration scalars are reused (1e-12 relative)
+            f.new_dt = 0;
+        } else {
+            f.new_dt = 1;
+        }
+    }
+    KKin &kin = c->kin;
+    kin.T = T;
+    for (int i = 0; i < 3; ++i) {
+        kin.alpha[i] = (double)fe.al[i];
+        kin.lam[i] = (double)fe.lam[i];
+    }
+    kin.beta0 = (double)fe.be[0];
+
+    const int Tp = round_up4(T);
+    cudaError_t e = cudaSuccess;
+#define TRY(x) if (e == cudaSuccess) e = (x)
+    TRY(dalloc(c, &c->d_fwd, (size_t)A));
+    TRY(dalloc(c, &c->d_bwd, (size_t)A));
+    TRY(dalloc(c, &c->d_frames, (size_t)T));
+    TRY(dalloc(c, &c->d_mask, (size_t)nx * ny));
+    TRY(dalloc(c, &c->d_sens, (size_t)(g.S + 1) * nx * ny));
+    TRY(dalloc(c, &c->d_smax, (size_t)g.S + 1));
+    TRY(dalloc(c, &c->d_tmp_smax, (size_t)1));
+    TRY(dalloc(c, &c->xi, c->n_pix_pad * Tp));
+    TRY(dalloc(c, &c->Fi, c->n_pix_pad * Tp));
+    TRY(dalloc(c, &c->qi, c->n_ray_all * Tp));
+    TRY(dalloc(c, &c->yi, c->n_ray_all * Tp));
+    TRY(dalloc(c, &c->r_pad, (size_t)KCS_MAX_FRAMES));
+    TRY(dalloc(c, &c->theta2, 4 * c->n_vox));
+    TRY(cudaMemcpyAsync(c->d_fwd, fw.data(), sizeof(double4) * A, cudaMemcpyHostToDevice, c->stream));
+    TRY(cudaMemcpyAsync(c->d_bwd, bw.data(), sizeof(double4) * A, cudaMemcpyHostToDevice, c->stream));
+    TRY(cudaMemcpyAsync(c->d_frames, frames.data(), sizeof(KFrame) * T, cudaMemcpyHostToDevice, c->stream));
+    TRY(cudaMemcpyAsync(c->d_mask, c->h_mask.data(), (size_t)nx * ny, cudaMemcpyHostToDevice, c->stream));
+    TRY(cudaMemsetAsync(c->Fi, 0, c->n_pix_pad * Tp * sizeof(float), c->stream));
+#undef TRY
+    if (e != cudaSuccess) {
+        const bool oom = (e == cudaErrorMemoryAllocation);
+        std::string msg = std::string("kcs_create: ") + cudaGetErrorString(e);
+        cudaGetLastError();
+        kcs_destroy(c);
+        return fail(nullptr, oom ? KCS_ERR_ALLOC : KCS_ERR_CUDA, msg);
+    }
+    g.fwd = c->d_fwd;
+    g.bwd = c->d_bwd;
+    kin.frames = c->d_frames;
+    rc = kcs_launch_sens(c);
+    if (rc == KCS_OK && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = KCS_ERR_CUDA;
+    if (rc != KCS_OK) {
+        std::string msg = "kcs_create: sensitivity kernel failed: " + c->err;
+        kcs_destroy(c);
+        return fail(nullptr, rc, msg);
+    }
+    *out = c;
+    return KCS_OK;
+}
+
+int kcs_forward_project(kcs_ctx *c, const float *x, float *y_s, int subset, int f0, int nf) {
+    if (!c) return KCS_ERR_NULL;
+    if (!x || !y_s) return fail(c, KCS_ERR_NULL, "kcs_forward_project: NULL buffer");
+    int rc = check_subset_frames(c, subset, f0, nf);
+    if (rc) return rc;
+    const KGeom &g = c->g;
+    const int Tp = round_up4(nf), As = subset < 0 ? g.A : g.A / g.S;
+    if ((rc = ensure_border(c, Tp))) return rc;
+    if ((rc = pack_image(c, x + (size_t)f0 * c->n_vox, nf, c->xi, Tp))) return rc;
+    if ((rc = kcs_launch_forward(c, Tp, subset, 0, 1.f, 0))) return rc;
+    return unpack_sino(c, c->qi, Tp, y_s + (size_t)f0 * g.nz * As * g.B, nf, As);
+}
+
+int kcs_back_project(kcs_ctx *c, const float *q_s, float *b, int subset, int f0, int nf) {
+    if (!c) return KCS_ERR_NULL;
+    if (!q_s || !b) return fail(c, KCS_ERR_NULL, "kcs_back_project: NULL buffer");
+    int rc = check_subset_frames(c, subset, f0, nf);
+    if (rc) return rc;
+    const KGeom &g = c->g;
+    const int Tp = round_up4(nf), As = subset < 0 ? g.A : g.A / g.S;
+    if ((rc = ensure_border(c, Tp))) return rc;
+    if ((rc = pack_sino(c, q_s + (size_t)f0 * g.nz * As * g.B, nf, c->qi, Tp, As))) return rc;
+    if ((rc = kcs_launch_back(c, Tp, subset, 0, c->xi, 1.f, 0.f))) return rc;
+    return unpack_image(c, c->xi, Tp, b + (size_t)f0 * c->n_vox, nf);
+}
+
+int kcs_sensitivity(kcs_ctx *c, int subset, float *sens) {
+    if (!c) return KCS_ERR_NULL;
+    if (!sens) return fail(c, KCS_ERR_NULL, "kcs_sensitivity: NULL buffer");
+    if (subset < -1 || subset >= c->g.S) return fail(c, KCS_ERR_SHAPE, "subset out of range");
+    const size_t v2 = (size_t)c->g.nx * c->g.ny;
+    const int sidx = subset < 0 ? c->g.S : subset;
+    KCS_CUDA_OK(c, cudaMemcpyAsync(sens, c->d_sens + sidx * v2, v2 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    return KCS_OK;
+}
+
+int kcs_osl_update(kcs_ctx *c, float *x, const float *bp, const float *sens, const float *F, float beta, int prior_mode,
+                   float sigma2) {
+    if (!c) return KCS_ERR_NULL;
+    if (!x || !bp || !sens || !F) return fail(c, KCS_ERR_NULL, "kcs_osl_update: NULL buffer");
+    if (prior_mode != KCS_PRIOR_POISSON_MATCHED && prior_mode != KCS_PRIOR_ABSOLUTE)
+        return fail(c, KCS_ERR_SHAPE, "kcs_osl_update: unknown prior_mode");
+    if (prior_mode == KCS_PRIOR_ABSOLUTE && !(sigma2 > 0.f)) return fail(c, KCS_ERR_SHAPE, "kcs_osl_update: sigma2 <= 0");
+    return kcs_launch_osl_planar(c, x, bp, sens, F, beta, prior_mode, sigma2);
+}
+
+int kcs_kinetic_eval(kcs_ctx *c, const float *theta, float *F, float *J) {
+    if (!c) return KCS_ERR_NULL;
+    if (!theta || !F) return fail(c, KCS_ERR_NULL, "kcs_kinetic_eval: NULL buffer");
+    return kcs_launch_kinetic(c, theta, F, J, 0, 0);
+}
+
+// n_steps Jacobi steps ping-ponging between the caller's theta and the context's second buffer.
+static int lm_steps(kcs_ctx *c, const float *x, int x_inner, int Tp, float *theta, float *lambda, float gamma, float delta,
+                    int n_steps, float *cost) {
+    float *cur = theta, *nxt = c->theta2;
+    for (int s = 0; s < n_steps; ++s) {
+        int rc = kcs_launch_lm_step(c, x, x_inner, Tp, cur, nxt, lambda, gamma, delta, (s == n_steps - 1) ? cost : nullptr);
+        if (rc) return rc;
+        float *t = cur; cur = nxt; nxt = t;
+    }
+    if (cur != theta)
+        KCS_CUDA_OK(c, cudaMemcpyAsync(theta, cur, 4 * c->n_vox * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    return KCS_OK;
+}
+
+int kcs_map_lm(kcs_ctx *c, const float *x, float *theta, float *lambda, float gamma, float delta, int n_steps, float *cost) {
+    if (!c) return KCS_ERR_NULL;
+    if (!x || !theta || !lambda) return fail(c, KCS_ERR_NULL, "kcs_map_lm: NULL buffer");
+    if (n_steps < 0 || !(delta >= 0.f) || !(gamma >= 0.f)) return fail(c, KCS_ERR_SHAPE, "kcs_map_lm: negative n_steps/gamma/delta");
+    return lm_steps(c, x, 0, 0, theta, lambda, gamma, delta, n_steps, cost);
+}
+
+int kcs_icm_run(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta, float *lambda,
+                float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter) {
+    if (!c) return KCS_ERR_NULL;
+    if (!y || !r || !x || !theta || !lambda) return fail(c, KCS_ERR_NULL, "kcs_icm: NULL buffer");
+    if (r_mode != KCS_R_PER_FRAME && r_mode != KCS_R_FULL) return fail(c, KCS_ERR_SHAPE, "kcs_icm: unknown r_mode");
+    if (n_lm < 0 || n_iter < 0 || !(scale > 0.f)) return fail(c, KCS_ERR_SHAPE, "kcs_icm: bad n_lm / n_iter / scale");
+    const KGeom &g = c->g;
+    const int T = c->cfg.n_frames, Tp = round_up4(T);
+    int rc;
+    if ((rc = ensure_border(c, Tp))) return rc;
+    if ((rc = pack_image(c, x, T, c->xi, Tp))) return rc;
+    if ((rc = pack_sino(c, y, T, c->yi, Tp, g.A))) return rc;
+    if (r_mode == KCS_R_PER_FRAME) {
+        KCS_CUDA_OK(c, cudaMemsetAsync(c->r_pad, 0, KCS_MAX_FRAMES * sizeof(float), c->stream));
+        KCS_CUDA_OK(c, cudaMemcpyAsync(c->r_pad, r, T * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    } else {
+        if (!c->ri) {
+            if (dalloc(c, &c->ri, c->n_ray_all * Tp) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(c, KCS_ERR_ALLOC, "kcs_icm: cannot allocate the packed randoms sinogram");
+            }
+        }
+        if ((rc = pack_sino(c, r, T, c->ri, Tp, g.A))) return rc;
+    }
+    for (int it = 0; it < n_iter; ++it) {
+        const float b = it == 0 ? beta_first : beta;
+        // F <- K(theta^{n-1}), held fixed during the pass ("one step late")
+        if ((rc = kcs_launch_kinetic(c, theta, c->Fi, nullptr, 1, Tp))) return rc;
+        for (int s = 0; s < g.S; ++s) {  // Q5: subsets in order 0..S-1
+            if ((rc = kcs_launch_forward(c, Tp, s, 1, scale, r_mode))) return rc;
+            if ((rc = kcs_launch_back(c, Tp, s, 1, nullptr, scale, b))) return rc;
+        }
+        if ((rc = lm_steps(c, c->xi, 1, Tp, theta, lambda, gamma, delta, n_lm, nullptr))) return rc;
+    }
+    return unpack_image(c, c->xi, Tp, x, T);
+}
+
+int kcs_icm_iteration(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta,
+                      float *lambda, float beta, float gamma, float delta, int n_lm) {
+    return kcs_icm_run(c, y, r, r_mode, scale, x, theta, lambda, beta, beta, gamma, delta, n_lm, 1);
+}
+
+int kcs_icm_run_host(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta,
+                     float *lambda, float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter) {
+    if (!c) return KCS_ERR_NULL;
+    if (!y || !r || !x || !theta || !lambda) return fail(c, KCS_ERR_NULL, "kcs_icm_run_host: NULL buffer");
+    if (r_mode != KCS_R_PER_FRAME && r_mode != KCS_R_FULL) return fail(c, KCS_ERR_SHAPE, "kcs_icm_run_host: unknown r_mode");
+    const int T = c->cfg.n_frames;
+    const size_t ny_ = (size_t)T * c->n_ray_all, nx_ = (size_t)T * c->n_vox;
+    const size_t nr = r_mode == KCS_R_PER_FRAME ? (size_t)T : ny_;
+    cudaError_t e = cudaSuccess;
+    if (!c->st_y) {
+        if (e == cudaSuccess) e = dalloc(c, &c->st_y, ny_);
+        if (e == cudaSuccess) e = dalloc(c, &c->st_x, nx_);
+        if (e == cudaSuccess) e = dalloc(c, &c->st_theta, 4 * c->n_vox);
+        if (e == cudaSuccess) e = dalloc(c, &c->st_lambda, c->n_vox);
+    }
+    if (e == cudaSuccess && c->st_r_elems < nr) {
+        if (c->st_r) cudaFree(c->st_r);
+        c->st_r = nullptr;
+        e = dalloc(c, &c->st_r, nr);
+        c->st_r_elems = e == cudaSuccess ? nr : 0;
+    }
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, KCS_ERR_ALLOC, std::string("kcs_icm_run_host: ") + cudaGetErrorString(e));
+    }
+    cudaStream_t st = c->stream;
+    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_y, y, ny_ * sizeof(float), cudaMemcpyHostToDevice, st));
+    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_r, r, nr * sizeof(float), cudaMemcpyHostToDevice, st));
+    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_x, x, nx_ * sizeof(float), cudaMemcpyHostToDevice, st));
+    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_theta, theta, 4 * c->n_vox * sizeof(float), cudaMemcpyHostToDevice, st));
+    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_lambda, lambda, c->n_vox * sizeof(float), cudaMemcpyHostToDevice, st));
+    int rc = kcs_icm_run(c, c->st_y, c->st_r, r_mode, scale, c->st_x, c->st_theta, c->st_lambda, beta_first, beta, gamma, delta,
+                         n_lm, n_iter);
+    if (rc) return rc;
+    KCS_CUDA_OK(c, cudaMemcpyAsync(x, c->st_x, nx_ * sizeof(float), cudaMemcpyDeviceToHost, st));
+    KCS_CUDA_OK(c, cudaMemcpyAsync(theta, c->st_theta, 4 * c->n_vox * sizeof(float), cudaMemcpyDeviceToHost, st));
+    KCS_CUDA_OK(c, cudaMemcpyAsync(lambda, c->st_lambda, c->n_vox * sizeof(float), cudaMemcpyDeviceToHost, st));
+    KCS_CUDA_OK(c, cudaStreamSynchronize(st));
+    return KCS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,135 @@
+// kcs_internal.cuh -- shared declarations of the CUDA path (not part of the C ABI; see include/kcs.h).
+// Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "../../include/kcs.h"
+
+// ---------------------------------------------------------------------------------------------
+// Geometry handed to kernels by value.
+//   padded image layout ("inner"):  xi[z][j+1][i+1][Tp]  on a (ny+2) x (nx+2) grid whose border is 0,
+//   so every bilinear tap of a sample with i0 in [-1, nx-1] is a plain load (P2: outside pixels are 0).
+//   sinogram layout ("inner"):      qi[z][la][b][Tp]
+// ---------------------------------------------------------------------------------------------
+struct KGeom {
+    int nx, ny, nz;
+    int nxp, nyp;      // nx+2, ny+2
+    int A, B, K, S;
+    float step_mm;
+    double cx, cy, cb, ck;  // (nx-1)/2, (ny-1)/2, (B-1)/2, (K-1)/2
+    // per-angle tables (device, double4 each):
+    //   fwd[a] = (bin cos/vx, -step sin/vx, bin sin/vy, step cos/vy):  fx = (b-cb) f.x + (k-ck) f.y + cx ; fy = (b-cb) f.z + (k-ck) f.w + cy
+    //   bwd[a] = (vx cos/bin, vy sin/bin, -vx sin/step, vy cos/step):  fb = (i-cx) g.x + (j-cy) g.y + cb ; fk = (i-cx) g.z + (j-cy) g.w + ck
+    const double4 *fwd;
+    const double4 *bwd;
+};
+
+// Per-frame kinetic tables (fp64, device).  "b" = value at a frame boundary t (index 0: t_start, 1: t_end).
+//   P0[i] = int_0^t e^{-l_i u} du (i = 0..2);  P1_0 = int_0^t u e^{-l_0 u} du;
+//   Pn[i-1][n-1] = int_0^t u^n e^{-l_i u} du for i = 1,2 and n = 1..4 (Taylor branch when a ~ l_i).
+struct KBoundary {
+    double t;
+    double P0[3];
+    double P1_0;
+    double Pn[2][4];
+};
+struct KFrame {
+    KBoundary b[2];
+    double dICp;  // int_frame Cp
+    double W0;    // int_frame int_0^t Cp  (the a = 0 member of the W family, K3)
+    double dt;    // t_end - t_start
+    int contiguous;  // t_start == previous frame's t_end (state carried over)
+    int new_dt;      // dt differs from the previous frame's (per-duration scalars must be recomputed)
+};
+struct KKin {
+    int T;
+    double alpha[3];  // K1: Cp(t) = sum (alpha_i + beta_i t) e^{-l_i t}; (alpha, beta) = (-A2-A3, A1), (A2, 0), (A3, 0)
+    double beta0;
+    double lam[3];
+    const KFrame *frames;  // device [T]
+};
+
+struct kcs_ctx {
+    kcs_config cfg;
+    std::vector<double> ts, te;
+    cudaStream_t stream;
+    std::string err;
+    long long launches;
+    long long ws_bytes;
+
+    KGeom g;
+    KKin kin;
+    double4 *d_fwd, *d_bwd;
+    KFrame *d_frames;
+    unsigned char *d_mask;            // [ny][nx]
+    std::vector<unsigned char> h_mask;
+    float *d_sens;                    // [S+1][ny][nx], unscaled A_s^T 1; entry S = all angles
+    float *d_smax;                    // [S+1] max over the image of d_sens[s]
+    float *d_tmp_smax;                // [1] scratch for kcs_osl_update
+
+    // workspace (inner layouts), sized for Tp = 32
+    size_t n_pix_pad;  // nz * nyp * nxp
+    size_t n_vox;      // nz * ny * nx
+    size_t n_ray_all;  // nz * A * B
+    float *xi;   // [n_pix_pad][Tp]
+    float *Fi;   // [n_pix_pad][Tp]
+    float *qi;   // [n_ray_all][Tp]  (subset or full sinogram being processed)
+    float *yi;   // [n_ray_all][Tp]  packed measured data
+    float *ri;   // [n_ray_all][Tp]  packed randoms (KCS_R_FULL), allocated lazily
+    float *r_pad;  // [32] per-frame randoms padded with 0
+    float *theta2;  // [4][n_vox] ping-pong buffer for the Jacobi LM steps
+    int xi_border_tp;  // Tp for which xi's zero border is valid (0 = unknown)
+
+    // device staging buffers of kcs_icm_run_host, allocated lazily
+    float *st_y, *st_r, *st_x, *st_theta, *st_lambda;
+    size_t st_r_elems;
+};
+
+#define KCS_CUDA_OK(ctx, call)                                                                  \
+    do {                                                                                        \
+        cudaError_t e__ = (call);                                                               \
+        if (e__ != cudaSuccess) {                                                               \
+            (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e__);                   \
+            return KCS_ERR_CUDA;                                                                \
+        }                                                                                       \
+    } while (0)
+
+static inline int round_up4(int n) { return (n + 3) & ~3; }
+
+// Frames-per-thread choice for a padded frame count Tp (multiple of 4): the largest of {16? no: 8, 12, 4}
+// that divides Tp, preferring 8 (register budget); FG = Tp / FPT lanes share one sample.
+static inline int choose_fpt(int Tp) {
+    if (Tp % 8 == 0) return 8;
+    if (Tp % 12 == 0) return 12;
+    return 4;
+}
+
+// ---- launchers (kcs_projector.cu) ----------------------------------------------------------------
+// planar [nf][rows][W] (frame stride fs elements)  ->  inner [dst_index(row, col)][Tp]; frames >= nf are written 0.
+//   dst_index = (row / rps) * slab + (row % rps) * rstride + off + col
+int kcs_launch_pack(kcs_ctx *c, const float *src, size_t fs, int nf, float *dst, int Tp, long long nrows, int W,
+                    int rps, long long slab, int rstride, int off);
+int kcs_launch_unpack(kcs_ctx *c, const float *src, int Tp, float *dst, size_t fs, int nf, long long nrows, int W,
+                      int rps, long long slab, int rstride, int off);
+// forward projection of c->xi (Tp frames) for `subset`; out = c->qi.
+//   ratio == 0:  qi = step * sum                      (kcs_forward_project)
+//   ratio == 1:  qi = y / (scale*step*sum + r), 0 where the denominator <= 1e-12   (O1)
+int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, int r_mode);
+// gather back-projection of c->qi for `subset`.
+//   osl == 0:  out_inner (padded layout) = step * sum                              (kcs_back_project)
+//   osl == 1:  c->xi <- OSL update with bp = scale*step*sum, sens = scale*A_s^T 1, F = c->Fi   (O2)
+int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, float scale, float beta);
+int kcs_launch_sens(kcs_ctx *c);  // fills d_sens, d_smax
+int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *sens, const float *F, float beta,
+                          int prior_mode, float sigma2);
+
+// ---- launchers (kcs_kinetic.cu) ------------------------------------------------------------------
+// F (and J) from theta.  inner == 0: F planar [T][V], J planar [4][T][V] or NULL;  inner == 1: F = padded inner layout, Tp.
+int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp);
+// one Jacobi LM step: reads theta_in, writes theta_out (all voxels; masked-out voxels are copied through).
+//   x_inner == 0: x planar [T][V];  x_inner == 1: x = c->xi padded inner layout with Tp.
+int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const float *theta_in, float *theta_out,
+                       float *lambda, float gamma, float delta, float *cost);
