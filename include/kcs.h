@@ -79,6 +79,21 @@ int kcs_get_mask(const kcs_ctx *ctx, unsigned char *mask_host_out);
 /* Count of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
 long long kcs_launch_count(const kcs_ctx *ctx);
 
+/* Optional per-kernel timing for the roofline report.  While enabled, every kernel launch of this
+ * context is bracketed by CUDA events on the context's stream.  kcs_profile_read SYNCHRONISES the stream, adds the
+ * elapsed milliseconds and launch counts since the previous read into ms[class] / count[class] ([host] arrays of
+ * n_classes >= KCS_PROFILE_NCLASS entries, overwritten) and clears the records.  Classes: */
+#define KCS_PROFILE_PACK 0     /* planar -> frame-innermost transposes */
+#define KCS_PROFILE_UNPACK 1   /* frame-innermost -> planar */
+#define KCS_PROFILE_KINETIC 2  /* model-curve evaluator (a1) */
+#define KCS_PROFILE_FORWARD 3  /* forward projector + fused Poisson ratio (a3, a4) */
+#define KCS_PROFILE_BACK 4     /* gather back-projector + fused OSL update (a5, a6) */
+#define KCS_PROFILE_LM 5       /* MAP-LM step (a8-a10) */
+#define KCS_PROFILE_OTHER 6    /* sensitivity images, stand-alone OSL update */
+#define KCS_PROFILE_NCLASS 7
+int kcs_profile_enable(kcs_ctx *ctx, int on);
+int kcs_profile_read(kcs_ctx *ctx, double *ms, long long *count, int n_classes);
+
 /* P1-P3, P5 (BJ north_star "ray-driven parallel-beam line integrals with bilinear
  * interpolation"):  y_s[f] = A_s x[f]  for frames f in [f0, f0+nf), all batched in one launch.
  *   (A x)[z,a,b] = step_mm * sum_k bilinear(x[z]; sample(a,b,k)), pixels outside the image are 0.

@@ -26,10 +26,11 @@ PRIOR_ABSOLUTE = 1
 R_PER_FRAME = 0
 R_FULL = 1
 MAX_FRAMES = 32
+PROFILE_CLASSES = ("pack", "unpack", "kinetic", "forward", "back", "lm", "other")
 
 # every symbol include/kcs.h declares (tests/test_abi.py checks the library exports each of them)
 EXPORTS = ["kcs_create", "kcs_destroy", "kcs_set_stream", "kcs_last_error", "kcs_workspace_bytes", "kcs_get_mask",
-           "kcs_launch_count", "kcs_forward_project", "kcs_back_project", "kcs_sensitivity", "kcs_osl_update",
+           "kcs_launch_count", "kcs_profile_enable", "kcs_profile_read", "kcs_forward_project", "kcs_back_project", "kcs_sensitivity", "kcs_osl_update",
            "kcs_kinetic_eval", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host"]
 
 
@@ -82,6 +83,8 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.kcs_launch_count.argtypes = [vp]
     lib.kcs_launch_count.restype = C.c_longlong
     lib.kcs_get_mask.argtypes = [vp, vp]
+    lib.kcs_profile_enable.argtypes = [vp, i]
+    lib.kcs_profile_read.argtypes = [vp, vp, vp, i]
     lib.kcs_forward_project.argtypes = [vp, fp, fp, i, i, i]
     lib.kcs_back_project.argtypes = [vp, fp, fp, i, i, i]
     lib.kcs_sensitivity.argtypes = [vp, i, fp]
@@ -167,6 +170,17 @@ class Context:
 
     def launch_count(self) -> int:
         return int(self._lib.kcs_launch_count(self._h))
+
+    def profile_enable(self, on: bool = True):
+        self._check(self._lib.kcs_profile_enable(self._h, int(bool(on))))
+
+    def profile_read(self) -> dict:
+        """{class name: (milliseconds, launches)} since the previous read (synchronises the stream)."""
+        ms = np.zeros(len(PROFILE_CLASSES), dtype=np.float64)
+        n = np.zeros(len(PROFILE_CLASSES), dtype=np.int64)
+        self._check(self._lib.kcs_profile_read(self._h, ms.ctypes.data_as(C.c_void_p), n.ctypes.data_as(C.c_void_p),
+                                               len(PROFILE_CLASSES)))
+        return {k: (float(ms[q]), int(n[q])) for q, k in enumerate(PROFILE_CLASSES)}
 
     def mask(self) -> np.ndarray:
         m = np.zeros((self.ny, self.nx), dtype=np.uint8)

@@ -164,6 +164,30 @@ int kcs_set_stream(kcs_ctx *ctx, void *stream) {
     return KCS_OK;
 }
 
+int kcs_profile_enable(kcs_ctx *c, int on) {
+    if (!c) return KCS_ERR_NULL;
+    c->prof_on = on != 0;
+    return KCS_OK;
+}
+
+int kcs_profile_read(kcs_ctx *c, double *ms, long long *count, int n_classes) {
+    if (!c) return KCS_ERR_NULL;
+    if (!ms || !count) return fail(c, KCS_ERR_NULL, "kcs_profile_read: NULL buffer");
+    if (n_classes < KCS_PROFILE_NCLASS) return fail(c, KCS_ERR_SHAPE, "kcs_profile_read: n_classes < KCS_PROFILE_NCLASS");
+    for (int q = 0; q < n_classes; ++q) { ms[q] = 0.0; count[q] = 0; }
+    KCS_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+    for (const KProfRec &r : c->prof_recs) {
+        float t = 0.f;
+        KCS_CUDA_OK(c, cudaEventElapsedTime(&t, r.a, r.b));
+        ms[r.cls] += (double)t;
+        count[r.cls] += 1;
+        c->prof_pool.push_back(r.a);
+        c->prof_pool.push_back(r.b);
+    }
+    c->prof_recs.clear();
+    return KCS_OK;
+}
+
 int kcs_get_mask(const kcs_ctx *ctx, unsigned char *out) {
     if (!ctx || !out) return KCS_ERR_NULL;
     std::memcpy(out, ctx->h_mask.data(), ctx->h_mask.size());
@@ -177,6 +201,8 @@ int kcs_destroy(kcs_ctx *c) {
                     c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
     for (void *p : ptrs)
         if (p) cudaFree(p);
+    for (const KProfRec &r : c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
     delete c;
     return KCS_OK;
 }
@@ -203,6 +229,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->stream = (cudaStream_t)stream;
     c->launches = 0;
     c->ws_bytes = 0;
+    c->prof_on = false;
     c->xi_border_tp = 0;
     c->d_fwd = c->d_bwd = nullptr; c->d_frames = nullptr; c->d_mask = nullptr;
     c->d_sens = c->d_smax = c->d_tmp_smax = nullptr;

@@ -52,8 +52,18 @@ struct KKin {
     const KFrame *frames;  // device [T]
 };
 
+// Kernel classes for the optional per-kernel timing (kcs_profile_*; bench.py's roofline object).
+enum { KCS_K_PACK = 0, KCS_K_UNPACK, KCS_K_KINETIC, KCS_K_FORWARD, KCS_K_BACK, KCS_K_LM, KCS_K_OTHER, KCS_K_NCLASS };
+struct KProfRec {
+    cudaEvent_t a, b;
+    int cls;
+};
+
 struct kcs_ctx {
     kcs_config cfg;
+    bool prof_on;
+    std::vector<KProfRec> prof_recs;     // recorded, not yet read
+    std::vector<cudaEvent_t> prof_pool;  // events free for reuse
     std::vector<double> ts, te;
     cudaStream_t stream;
     std::string err;
@@ -96,6 +106,33 @@ struct kcs_ctx {
             return KCS_ERR_CUDA;                                                                \
         }                                                                                       \
     } while (0)
+
+// Brackets the launches of one kernel class with CUDA events on the context's stream when profiling is on.
+struct ProfScope {
+    kcs_ctx *c;
+    KProfRec r;
+    bool live;
+    static cudaEvent_t get(kcs_ctx *c) {
+        if (!c->prof_pool.empty()) {
+            cudaEvent_t e = c->prof_pool.back();
+            c->prof_pool.pop_back();
+            return e;
+        }
+        cudaEvent_t e = nullptr;
+        cudaEventCreate(&e);
+        return e;
+    }
+    ProfScope(kcs_ctx *ctx, int cls) : c(ctx), live(ctx->prof_on) {
+        if (!live) return;
+        r.a = get(c); r.b = get(c); r.cls = cls;
+        cudaEventRecord(r.a, c->stream);
+    }
+    ~ProfScope() {
+        if (!live) return;
+        cudaEventRecord(r.b, c->stream);
+        c->prof_recs.push_back(r);
+    }
+};
 
 static inline int round_up4(int n) { return (n + 3) & ~3; }
 

@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(128) k_lm_step(KGeom g, KKin kin, const float 
         for (int q = 0; q < nn; ++q)
 #pragma unroll
             for (int p = 0; p < 4; ++p) phi_new += gamma * huber(xt[p] - nb[q][p], delta);
-        if (phi_new <= phi_old) {
+        if (phi_new <= phi_old * (1.0 + 1e-6)) {  // Q15a: relative slack, see DESIGN.md section 3
 #pragma unroll
             for (int p = 0; p < 4; ++p) xi[p] = xt[p];
             lam = fmax(lam / 10.0, 1e-30);
@@ -338,6 +338,7 @@ __global__ void __launch_bounds__(128) k_lm_step(KGeom g, KKin kin, const float 
 int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp) {
     const long long nvox = (long long)c->n_vox;
     const size_t smem = sizeof(KFrame) * c->kin.T;
+    ProfScope ps(c, KCS_K_KINETIC);
     k_kinetic<<<(unsigned)((nvox + 127) / 128), 128, smem, c->stream>>>(c->g, c->kin, theta, F, J, nvox, inner, Tp);
     LAUNCH_CHECK(c);
     return KCS_OK;
@@ -347,6 +348,7 @@ int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const fl
                        float *lambda, float gamma, float delta, float *cost) {
     const long long nvox = (long long)c->n_vox;
     const size_t smem = sizeof(KFrame) * c->kin.T;
+    ProfScope ps(c, KCS_K_LM);
     k_lm_step<<<(unsigned)((nvox + 127) / 128), 128, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, theta_in, theta_out,
                                                                         lambda, c->d_mask, nvox, (double)gamma,
                                                                         (double)delta, cost);

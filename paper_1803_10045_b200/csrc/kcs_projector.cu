@@ -86,6 +86,7 @@ int kcs_launch_pack(kcs_ctx *c, const float *src, size_t fs, int nf, float *dst,
     PackMap m{nrows, W, rps, slab, rstride, off};
     dim3 grid;
     pack_grid(nrows, W, grid);
+    ProfScope ps(c, KCS_K_PACK);
     k_pack<<<grid, dim3(32, 8), 0, c->stream>>>(src, fs, nf, dst, Tp, m);
     LAUNCH_CHECK(c);
     return KCS_OK;
@@ -96,6 +97,7 @@ int kcs_launch_unpack(kcs_ctx *c, const float *src, int Tp, float *dst, size_t f
     PackMap m{nrows, W, rps, slab, rstride, off};
     dim3 grid;
     pack_grid(nrows, W, grid);
+    ProfScope ps(c, KCS_K_UNPACK);
     k_unpack<<<grid, dim3(32, 8), 0, c->stream>>>(src, Tp, dst, fs, nf, m);
     LAUNCH_CHECK(c);
     return KCS_OK;
@@ -245,6 +247,7 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
     const int threads = p.FG * bins * ks;
     const size_t smem = ks > 1 ? (size_t)(ks - 1) * FPT * bins * p.FG * sizeof(float) : 0;
     dim3 grid((g.B + bins - 1) / bins, p.As, g.nz);
+    ProfScope ps(c, KCS_K_FORWARD);
     switch (FPT) {
         case 4: k_forward<4><<<grid, threads, smem, c->stream>>>(g, p); break;
         case 8: k_forward<8><<<grid, threads, smem, c->stream>>>(g, p); break;
@@ -409,6 +412,13 @@ __global__ void __launch_bounds__(256) k_back(KGeom g, BackArgs p) {
 
 template <int FPT>
 static void back_dispatch(int ZB, dim3 grid, int threads, size_t smem, cudaStream_t st, const KGeom &g, const BackArgs &p) {
+    static bool optin = false;  // the weight chunk can exceed the 48 KB default (64 KB at 256 voxels per block)
+    if (!optin) {
+        cudaFuncSetAttribute(k_back<FPT, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+        cudaFuncSetAttribute(k_back<FPT, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+        cudaFuncSetAttribute(k_back<FPT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+        optin = true;
+    }
     switch (ZB) {
         case 4: k_back<FPT, 4><<<grid, threads, smem, st>>>(g, p); break;
         case 2: k_back<FPT, 2><<<grid, threads, smem, st>>>(g, p); break;
@@ -444,6 +454,7 @@ int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, f
     if (FPT == 12 && ZB == 4) ZB = 2;  // register budget
     dim3 grid(gx, gy, (g.nz + ZB - 1) / ZB);
     const size_t smem = (size_t)KCS_BACK_ACH * nvox * sizeof(float4);
+    ProfScope ps(c, KCS_K_BACK);
     switch (FPT) {
         case 4: back_dispatch<4>(ZB, grid, threads, smem, c->stream, g, p); break;
         case 8: back_dispatch<8>(ZB, grid, threads, smem, c->stream, g, p); break;
@@ -478,6 +489,7 @@ int kcs_launch_sens(kcs_ctx *c) {
     cudaError_t e = cudaMemsetAsync(c->d_smax, 0, sizeof(float) * (g.S + 1), c->stream);
     if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return KCS_ERR_CUDA; }
     dim3 grid((g.nx + 127) / 128, g.ny, g.S + 1);
+    ProfScope ps(c, KCS_K_OTHER);
     k_sens<<<grid, 128, 0, c->stream>>>(g, c->d_sens, c->d_smax);
     LAUNCH_CHECK(c);
     return KCS_OK;
@@ -519,6 +531,7 @@ int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *se
     const int v2 = g.nx * g.ny;
     cudaError_t e = cudaMemsetAsync(c->d_tmp_smax, 0, sizeof(float), c->stream);
     if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return KCS_ERR_CUDA; }
+    ProfScope ps(c, KCS_K_OTHER);
     k_max_nonneg<<<64, 256, 0, c->stream>>>(sens, v2, c->d_tmp_smax);
     LAUNCH_CHECK(c);
     const size_t n = (size_t)c->cfg.n_frames * c->n_vox;

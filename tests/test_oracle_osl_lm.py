@@ -130,7 +130,7 @@ def test_cost_nonincreasing_and_jacobi_order():
         b_th, b_lam = o.map_lm(x, b_th, b_lam, gamma, delta, 1)
     np.testing.assert_array_equal(a_th, b_th)
     np.testing.assert_array_equal(a_lam, b_lam)
-    # Phi_v with neighbours frozen at the step's start never increases within a step
+    # Phi_v with neighbours frozen at the step's start never increases within a step (beyond the 1e-6 slack of Q15a)
     prev_th, prev_lam = cur, lam
     for _ in range(4):
         new_th, new_lam, cost = o.map_lm(x, prev_th, prev_lam, gamma, delta, 1, want_cost=True)
@@ -139,7 +139,7 @@ def test_cost_nonincreasing_and_jacobi_order():
                   if mask[j + dj, i + di]]
             before = o.lm_objective(x[:, 0, j, i], prev_th[:, 0, j, i], nb, gamma, delta)
             after = o.lm_objective(x[:, 0, j, i], new_th[:, 0, j, i], nb, gamma, delta)
-            assert after <= before * (1 + 1e-14)
+            assert after <= before * (1 + 1e-6)
             assert abs(after - cost[0, j, i]) <= 1e-12 * max(1.0, abs(after))
         prev_th, prev_lam = new_th, new_lam
 
