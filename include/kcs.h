@@ -94,6 +94,14 @@ long long kcs_launch_count(const kcs_ctx *ctx);
 int kcs_profile_enable(kcs_ctx *ctx, int on);
 int kcs_profile_read(kcs_ctx *ctx, double *ms, long long *count, int n_classes);
 
+/* Machine-peak microbenchmarks for the roofline denominators that MEASURED_PEAKS.json lacks:
+ * runs a small kernel on the context's stream (best of 5, CUDA events), SYNCHRONISES, and writes *out [host]. */
+#define KCS_PEAK_FP32_TFLOPS 0 /* dependent-free FFMA chains, 2 flop per FMA */
+#define KCS_PEAK_FP64_TFLOPS 1 /* the same with DFMA */
+#define KCS_PEAK_L2_GBS 2      /* L2-resident 32 MB buffer streamed by every CTA with ld.global.cg */
+#define KCS_PEAK_L1_GBS 3      /* 16 KB window per CTA re-read with coalesced LDG.128 (L1 hits) */
+int kcs_probe_peak(kcs_ctx *ctx, int what, double *out);
+
 /* P1-P3, P5 (BJ north_star "ray-driven parallel-beam line integrals with bilinear
  * interpolation"):  y_s[f] = A_s x[f]  for frames f in [f0, f0+nf), all batched in one launch.
  *   (A x)[z,a,b] = step_mm * sum_k bilinear(x[z]; sample(a,b,k)), pixels outside the image are 0.

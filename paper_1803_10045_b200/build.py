@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkcs.so")
-SOURCES = ["kcs_api.cu", "kcs_projector.cu", "kcs_kinetic.cu"]
+SOURCES = ["kcs_api.cu", "kcs_projector.cu", "kcs_kinetic.cu", "kcs_probe.cu"]
 HEADERS = [os.path.join(CSRC, "kcs_internal.cuh"), os.path.join(HERE, "..", "include", "kcs.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -1,0 +1,138 @@
+// kcs_probe.cu -- machine-peak microbenchmarks behind kcs_probe_peak (include/kcs.h).
+//
+// MEASURED_PEAKS.json holds an HBM copy figure and a bf16 GEMM figure only; the rooflines that bound
+// this path (FP32 / FP64 FMA issue, L2->SM bandwidth, L1 bandwidth) must be measured on the box, in the same run
+// as the kernels they normalise.  Each probe is timed with CUDA events on the context's stream (best of 5).
+#include "kcs_internal.cuh"
+
+namespace {
+
+template <class R>
+__global__ void __launch_bounds__(256) k_fma_peak(R *out, int iters, R seed) {
+    // 8 independent chains per thread: enough ILP to hide the 4-cycle FMA latency at 8 warps per scheduler
+    R a0 = seed + (R)threadIdx.x, a1 = a0 + (R)1, a2 = a0 + (R)2, a3 = a0 + (R)3;
+    R a4 = a0 + (R)4, a5 = a0 + (R)5, a6 = a0 + (R)6, a7 = a0 + (R)7;
+    const R m = (R)0.999, c = (R)0.001;
+#pragma unroll 4
+    for (int i = 0; i < iters; ++i) {
+        a0 = a0 * m + c; a1 = a1 * m + c; a2 = a2 * m + c; a3 = a3 * m + c;
+        a4 = a4 * m + c; a5 = a5 * m + c; a6 = a6 * m + c; a7 = a7 * m + c;
+    }
+    const R s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == (R)-12345) out[0] = s;  // never true; keeps the chains alive
+}
+
+// Every CTA streams the whole `n4`-float4 buffer (L2 resident) with .cg loads, starting at a different offset.
+__global__ void __launch_bounds__(256) k_l2_read(const float4 *__restrict__ buf, size_t n4, int reps, float *out) {
+    float s = 0.f;
+    const size_t start = ((size_t)blockIdx.x * 9973u * 256u) % n4;
+    for (int r = 0; r < reps; ++r) {
+        size_t q = start + threadIdx.x;
+        for (size_t e = threadIdx.x; e < n4; e += 256 * 4) {
+            // 4 independent loads in flight per thread
+            float4 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                size_t p = q + (size_t)u * 256;
+                if (p >= n4) p -= n4;
+                v[u] = __ldcg(buf + p);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) s += v[u].x + v[u].y + v[u].z + v[u].w;
+            q += 256 * 4;
+            if (q >= n4) q -= n4;
+        }
+    }
+    if (s == -12345.f) out[0] = s;
+}
+
+// Every warp re-reads its CTA's 16 KB window with fully coalesced LDG.128 (4 lines of 128 B per instruction): L1 hits.
+__global__ void __launch_bounds__(256) k_l1_read(const float4 *__restrict__ buf, int iters, float *out) {
+    const float4 *w = buf + (size_t)blockIdx.x * 1024;  // 16 KB per CTA
+    float s = 0.f;
+    int p = threadIdx.x;
+    for (int i = 0; i < iters; ++i) {
+        float4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = __ldg(w + ((p + u * 256) & 1023));
+#pragma unroll
+        for (int u = 0; u < 4; ++u) s += v[u].x + v[u].y + v[u].z + v[u].w;
+        p = (p + 32) & 1023;
+    }
+    if (s == -12345.f) out[0] = s;
+}
+
+template <class Launch>
+int best_ms(kcs_ctx *c, Launch launch, float &best) {
+    cudaEvent_t a, b;
+    KCS_CUDA_OK(c, cudaEventCreate(&a));
+    KCS_CUDA_OK(c, cudaEventCreate(&b));
+    best = 1e30f;
+    for (int rep = 0; rep < 6; ++rep) {  // first repetition warms up
+        cudaEventRecord(a, c->stream);
+        launch();
+        cudaEventRecord(b, c->stream);
+        cudaError_t e = cudaEventSynchronize(b);
+        if (e != cudaSuccess) {
+            c->err = std::string("kcs_probe_peak: ") + cudaGetErrorString(e);
+            cudaEventDestroy(a); cudaEventDestroy(b);
+            return KCS_ERR_CUDA;
+        }
+        float t = 0.f;
+        cudaEventElapsedTime(&t, a, b);
+        if (rep > 0 && t < best) best = t;
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    return KCS_OK;
+}
+
+}  // namespace
+
+extern "C" int kcs_probe_peak(kcs_ctx *c, int what, double *out) {
+    if (!c) return KCS_ERR_NULL;
+    if (!out) { c->err = "kcs_probe_peak: NULL out"; return KCS_ERR_NULL; }
+    int dev = 0, sms = 0;
+    KCS_CUDA_OK(c, cudaGetDevice(&dev));
+    KCS_CUDA_OK(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int grid = sms * 8;  // 8 CTAs of 256 threads per SM = 2048 resident threads
+    float *scratch = nullptr;
+    const size_t l2_bytes = 32u << 20;  // well inside the 126 MB L2, far beyond the 256 KB L1s
+    KCS_CUDA_OK(c, cudaMalloc((void **)&scratch, l2_bytes));
+    cudaMemsetAsync(scratch, 0, l2_bytes, c->stream);
+    float ms = 0.f;
+    int rc = KCS_OK;
+    switch (what) {
+        case KCS_PEAK_FP32_TFLOPS: {
+            const int iters = 1 << 14;
+            rc = best_ms(c, [&] { k_fma_peak<float><<<grid, 256, 0, c->stream>>>(scratch, iters, 1.0f); }, ms);
+            *out = 2.0 * 8.0 * iters * 256.0 * grid / (ms * 1e-3) * 1e-12;
+            break;
+        }
+        case KCS_PEAK_FP64_TFLOPS: {
+            const int iters = 1 << 13;
+            rc = best_ms(c, [&] { k_fma_peak<double><<<grid, 256, 0, c->stream>>>((double *)scratch, iters, 1.0); }, ms);
+            *out = 2.0 * 8.0 * iters * 256.0 * grid / (ms * 1e-3) * 1e-12;
+            break;
+        }
+        case KCS_PEAK_L2_GBS: {
+            const int reps = 4;
+            const size_t n4 = l2_bytes / 16;
+            rc = best_ms(c, [&] { k_l2_read<<<sms * 4, 256, 0, c->stream>>>((const float4 *)scratch, n4, reps, scratch); }, ms);
+            *out = (double)l2_bytes * reps * (sms * 4) / (ms * 1e-3) * 1e-9;
+            break;
+        }
+        case KCS_PEAK_L1_GBS: {
+            const int iters = 1 << 12;
+            rc = best_ms(c, [&] { k_l1_read<<<grid, 256, 0, c->stream>>>((const float4 *)scratch, iters, scratch); }, ms);
+            *out = 16.0 * 4.0 * iters * 256.0 * grid / (ms * 1e-3) * 1e-9;
+            break;
+        }
+        default:
+            c->err = "kcs_probe_peak: unknown probe";
+            rc = KCS_ERR_SHAPE;
+    }
+    c->launches += (rc == KCS_OK) ? 6 : 0;
+    cudaFree(scratch);
+    return rc;
+}
