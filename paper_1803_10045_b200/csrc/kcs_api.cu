@@ -126,12 +126,12 @@ int ensure_border(kcs_ctx *c, int Tp) {
 int pack_image(kcs_ctx *c, const float *planar, int nf, float *inner, int Tp) {
     const KGeom &g = c->g;
     return kcs_launch_pack(c, planar, c->n_vox, nf, inner, Tp, (long long)g.nz * g.ny, g.nx, g.ny,
-                           (long long)g.nyp * g.nxp, g.nxp, g.nxp + 1);
+                           (long long)g.nyp * g.nxp, g.nxp, KCS_PAD * (g.nxp + 1));
 }
 int unpack_image(kcs_ctx *c, const float *inner, int Tp, float *planar, int nf) {
     const KGeom &g = c->g;
     return kcs_launch_unpack(c, inner, Tp, planar, c->n_vox, nf, (long long)g.nz * g.ny, g.nx, g.ny,
-                             (long long)g.nyp * g.nxp, g.nxp, g.nxp + 1);
+                             (long long)g.nyp * g.nxp, g.nxp, KCS_PAD * (g.nxp + 1));
 }
 int pack_sino(kcs_ctx *c, const float *planar, int nf, float *inner, int Tp, int As) {
     const KGeom &g = c->g;
@@ -197,7 +197,7 @@ int kcs_get_mask(const kcs_ctx *ctx, unsigned char *out) {
 int kcs_destroy(kcs_ctx *c) {
     if (!c) return KCS_ERR_NULL;
     cudaStreamSynchronize(c->stream);
-    void *ptrs[] = {c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->xi, c->Fi,
+    void *ptrs[] = {c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->d_wtab, c->xi, c->Fi,
                     c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
     for (void *p : ptrs)
         if (p) cudaFree(p);
@@ -233,13 +233,14 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->xi_border_tp = 0;
     c->d_fwd = c->d_bwd = nullptr; c->d_frames = nullptr; c->d_mask = nullptr;
     c->d_sens = c->d_smax = c->d_tmp_smax = nullptr;
+    c->d_wtab = nullptr;
     c->xi = c->Fi = c->qi = c->yi = c->ri = c->r_pad = c->theta2 = nullptr;
     c->st_y = c->st_r = c->st_x = c->st_theta = c->st_lambda = nullptr;
     c->st_r_elems = 0;
 
     const int nx = cfg->nx, ny = cfg->ny, nz = cfg->nz, A = cfg->n_angles, B = cfg->n_bins, K = cfg->n_steps, T = cfg->n_frames;
     KGeom &g = c->g;
-    g.nx = nx; g.ny = ny; g.nz = nz; g.nxp = nx + 2; g.nyp = ny + 2;
+    g.nx = nx; g.ny = ny; g.nz = nz; g.nxp = nx + 2 * KCS_PAD; g.nyp = ny + 2 * KCS_PAD;
     g.A = A; g.B = B; g.K = K; g.S = cfg->n_subsets;
     g.step_mm = cfg->step_mm;
     g.cx = 0.5 * (nx - 1); g.cy = 0.5 * (ny - 1); g.cb = 0.5 * (B - 1); g.ck = 0.5 * (K - 1);
@@ -307,6 +308,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     kin.beta0 = (double)fe.be[0];
 
     const int Tp = round_up4(T);
+    c->nbi = (nx + 1) / 2; c->nbj = (ny + 1) / 2; c->nbi4 = (c->nbi + 3) / 4;
     cudaError_t e = cudaSuccess;
 #define TRY(x) if (e == cudaSuccess) e = (x)
     TRY(dalloc(c, &c->d_fwd, (size_t)A));
@@ -316,6 +318,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     TRY(dalloc(c, &c->d_sens, (size_t)(g.S + 1) * nx * ny));
     TRY(dalloc(c, &c->d_smax, (size_t)g.S + 1));
     TRY(dalloc(c, &c->d_tmp_smax, (size_t)1));
+    TRY(dalloc(c, &c->d_wtab, (size_t)A * c->nbj * c->nbi4 * 24));
     TRY(dalloc(c, &c->xi, c->n_pix_pad * Tp));
     TRY(dalloc(c, &c->Fi, c->n_pix_pad * Tp));
     TRY(dalloc(c, &c->qi, c->n_ray_all * Tp));
@@ -339,6 +342,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     g.bwd = c->d_bwd;
     kin.frames = c->d_frames;
     rc = kcs_launch_sens(c);
+    if (rc == KCS_OK) rc = kcs_launch_build_wtab(c);
     if (rc == KCS_OK && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = KCS_ERR_CUDA;
     if (rc != KCS_OK) {
         std::string msg = "kcs_create: sensitivity kernel failed: " + c->err;

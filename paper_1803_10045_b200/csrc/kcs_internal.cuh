@@ -10,13 +10,16 @@
 
 // ---------------------------------------------------------------------------------------------
 // Geometry handed to kernels by value.
-//   padded image layout ("inner"):  xi[z][j+1][i+1][Tp]  on a (ny+2) x (nx+2) grid whose border is 0,
-//   so every bilinear tap of a sample with i0 in [-1, nx-1] is a plain load (P2: outside pixels are 0).
+//   padded image layout ("inner"):  xi[z][j+PAD][i+PAD][Tp]  on a (ny+2 PAD) x (nx+2 PAD) grid whose border is 0,
+//   so every bilinear tap of a sample with i0 in [-2, nx] is a plain load (P2: outside pixels are 0); the second
+//   border pixel lets the forward projector clip rays with a half-pixel margin instead of testing every sample.
 //   sinogram layout ("inner"):      qi[z][la][b][Tp]
 // ---------------------------------------------------------------------------------------------
+#define KCS_PAD 2  // zero pixels around every slice of the padded layout
+
 struct KGeom {
     int nx, ny, nz;
-    int nxp, nyp;      // nx+2, ny+2
+    int nxp, nyp;      // nx + 2 KCS_PAD, ny + 2 KCS_PAD
     int A, B, K, S;
     float step_mm;
     double cx, cy, cb, ck;  // (nx-1)/2, (ny-1)/2, (B-1)/2, (K-1)/2
@@ -79,6 +82,8 @@ struct kcs_ctx {
     float *d_sens;                    // [S+1][ny][nx], unscaled A_s^T 1; entry S = all angles
     float *d_smax;                    // [S+1] max over the image of d_sens[s]
     float *d_tmp_smax;                // [1] scratch for kcs_osl_update
+    float4 *d_wtab;                   // back-projector weight table [A][nbj][nbi4][6][4] (k_build_wtab)
+    int nbi, nbj, nbi4;               // 2x2 voxel blocks in x, y; groups of 4 blocks in x
 
     // workspace (inner layouts), sized for Tp = 32
     size_t n_pix_pad;  // nz * nyp * nxp
@@ -161,6 +166,7 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
 //   osl == 1:  c->xi <- OSL update with bp = scale*step*sum, sens = scale*A_s^T 1, F = c->Fi   (O2)
 int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, float scale, float beta);
 int kcs_launch_sens(kcs_ctx *c);  // fills d_sens, d_smax
+int kcs_launch_build_wtab(kcs_ctx *c);  // fills d_wtab
 int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *sens, const float *F, float beta,
                           int prior_mode, float sigma2);
 

@@ -169,7 +169,7 @@ __device__ __forceinline__ XAddr x_addr(const KGeom &g, size_t nvox, long long v
         const int v2 = g.nx * g.ny;
         const int z = (int)(v / v2), rem = (int)(v - (long long)z * v2);
         const int j = rem / g.nx, i = rem - j * g.nx;
-        r.base = (((size_t)z * g.nyp + (j + 1)) * g.nxp + (i + 1)) * Tp;
+        r.base = (((size_t)z * g.nyp + (j + KCS_PAD)) * g.nxp + (i + KCS_PAD)) * Tp;
         r.fstride = 1;
     }
     return r;

@@ -8,6 +8,7 @@
 // ray sample (forward) or one voxel (backward); each lane owns FPT frames as float4 registers.  Geometry math is
 // frame-independent and amortised over the FPT frames; coalescing comes from the frame axis and therefore does
 // not depend on the projection angle.
+#include <cstdlib>
 #include "kcs_internal.cuh"
 
 #define LAUNCH_CHECK(c)                                                     \
@@ -112,7 +113,7 @@ struct FwdArgs {
     const float *yi;     // packed measured sinogram [nz][A][B][Tp]       (ratio only)
     const float *ri;     // packed randoms, same layout                    (ratio, KCS_R_FULL)
     const float *r_pad;  // [32] per-frame randoms, 0 beyond T             (ratio, KCS_R_PER_FRAME)
-    int Tp, FG, BINS, KSPLIT, KCH;
+    int Tp, FG, BINS, KSPLIT, KCH, FB;
     int As, subset;
     int ratio, r_mode;
     float scale;
@@ -120,13 +121,15 @@ struct FwdArgs {
 
 #define KCS_ANCHOR 16  // steps between fp64 re-anchoring of the sample coordinates
 
-template <int FPT>
+// One thread = one ray x 4 frames; the FG = Tp/4 lanes of a ray read a whole pixel (16 FG bytes) per tap in one request.
+template <int FG>
 __global__ void __launch_bounds__(256) k_forward(KGeom g, FwdArgs p) {
+    constexpr int FPT = 4, Tp = 4 * FG;
     extern __shared__ float red[];
     const int tid = threadIdx.x;
-    const int fg = tid % p.FG;
-    const int bl = (tid / p.FG) % p.BINS;
-    const int kc = tid / (p.FG * p.BINS);
+    const int fg = tid % FG;
+    const int bl = (tid / FG) % p.BINS;
+    const int kc = tid / (FG * p.BINS);
     const int b = blockIdx.x * p.BINS + bl;
     const int la = blockIdx.y, z = blockIdx.z;
     const int a = p.subset < 0 ? la : p.subset + la * g.S;
@@ -138,50 +141,60 @@ __global__ void __launch_bounds__(256) k_forward(KGeom g, FwdArgs p) {
     if (b < g.B) {
         const double4 fw = g.fwd[a];
         const double bc = (double)b - g.cb;
-        const float dxk = (float)fw.y, dyk = (float)fw.w;
-        const int k_lo = kc * p.KCH;
-        const int k_hi = min(g.K, k_lo + p.KCH);
-        const int Tp = p.Tp;
+        // Sample coordinates advance along the ray as 32-bit fixed point with FB fractional bits (2^-22 pixel at
+        // image sizes <= 480), re-anchored from fp64 every KCS_ANCHOR steps: floor = shift, fraction = mask, and the
+        // fraction becomes a float by placing it in the mantissa of [1,2) -- no conversions, no floorf.  The bilinear
+        // interpolant is continuous (P2), so the <= 2e-6 pixel drift inside a block only perturbs the value by O(eps).
+        const int FB = p.FB, msh = 23 - FB;
+        const double qs = (double)(1 << FB);
+        const int dxq = __double2int_rn(fw.y * qs), dyq = __double2int_rn(fw.w * qs);
+        const unsigned fmask = (1u << FB) - 1u;
+        // Ray clipping: padded coordinates P = index + KCS_PAD.  A sample contributes iff floor(P) in [PAD-1, PAD+n-1];
+        // the loop runs over the k with P in [PAD - 1.5, PAD + n + 0.5) in both axes (a half-pixel margin that dwarfs the
+        // fixed-point drift): every tap of such a sample lies inside the padded slice and the extra samples read zeros.
+        const double pxa = fma(-g.ck, fw.y, fma(bc, fw.x, g.cx + (double)KCS_PAD));  // P_x at k = 0
+        const double pya = fma(-g.ck, fw.w, fma(bc, fw.z, g.cy + (double)KCS_PAD));
+        double tlo = (double)(kc * p.KCH), thi = (double)(min(g.K, (kc + 1) * p.KCH) - 1);
+        {
+            const double lo = (double)KCS_PAD - 1.5, hx = (double)(KCS_PAD + g.nx) + 0.5, hy = (double)(KCS_PAD + g.ny) + 0.5;
+            if (fabs(fw.y) < 1e-9) { if (!(pxa >= lo && pxa < hx)) thi = -1.0; }
+            else { const double t0 = (lo - pxa) / fw.y, t1 = (hx - pxa) / fw.y; tlo = fmax(tlo, fmin(t0, t1) + 1e-6); thi = fmin(thi, fmax(t0, t1) - 1e-6); }
+            if (fabs(fw.w) < 1e-9) { if (!(pya >= lo && pya < hy)) thi = -1.0; }
+            else { const double t0 = (lo - pya) / fw.w, t1 = (hy - pya) / fw.w; tlo = fmax(tlo, fmin(t0, t1) + 1e-6); thi = fmin(thi, fmax(t0, t1) - 1e-6); }
+        }
+        const int k_lo = (int)ceil(tlo);       // clip bounds were moved 1e-6 steps inwards: strictly inside the margin
+        const int k_hi = (int)floor(thi) + 1;
         const int rowstride = g.nxp * Tp;
         const float *slice = p.xi + (size_t)z * g.nyp * rowstride + fg * FPT;
         for (int k0 = k_lo; k0 < k_hi; k0 += KCS_ANCHOR) {
-            // fp64 anchor (P2): padded continuous index of sample (b, k0); integer part kept as int, fraction as fp32
-            const double kk = (double)k0 - g.ck;
-            const double px0 = fma(kk, fw.y, fma(bc, fw.x, g.cx + 1.0));
-            const double py0 = fma(kk, fw.w, fma(bc, fw.z, g.cy + 1.0));
-            const double flx0 = floor(px0), fly0 = floor(py0);
-            const int ia = (int)flx0, ja = (int)fly0;
-            const float fax = (float)(px0 - flx0), fay = (float)(py0 - fly0);
+            // fp64 anchor (P2): padded continuous index of sample (b, k0)
+            const double kk = (double)k0;
+            int fxq = __double2int_rn(fma(kk, fw.y, pxa) * qs), fyq = __double2int_rn(fma(kk, fw.w, pya) * qs);
             const int mmax = min(KCS_ANCHOR, k_hi - k0);
+#pragma unroll 4
             for (int m = 0; m < mmax; ++m) {
-                const float fxm = fmaf((float)m, dxk, fax), fym = fmaf((float)m, dyk, fay);
-                const float flx = floorf(fxm), fly = floorf(fym);
-                const float wx = fxm - flx, wy = fym - fly;
-                const int i0 = ia + (int)flx, j0 = ja + (int)fly;
-                if ((unsigned)i0 <= (unsigned)g.nx && (unsigned)j0 <= (unsigned)g.ny) {
-                    const float *p00 = slice + (size_t)j0 * rowstride + i0 * Tp;
-                    const float w00 = (1.f - wx) * (1.f - wy), w10 = wx * (1.f - wy);
-                    const float w01 = (1.f - wx) * wy, w11 = wx * wy;
-#pragma unroll
-                    for (int q = 0; q < FPT / 4; ++q) {
-                        const float4 v00 = __ldg(reinterpret_cast<const float4 *>(p00) + q);
-                        const float4 v10 = __ldg(reinterpret_cast<const float4 *>(p00 + Tp) + q);
-                        const float4 v01 = __ldg(reinterpret_cast<const float4 *>(p00 + rowstride) + q);
-                        const float4 v11 = __ldg(reinterpret_cast<const float4 *>(p00 + rowstride + Tp) + q);
-                        acc[4 * q + 0] += w00 * v00.x + w10 * v10.x + w01 * v01.x + w11 * v11.x;
-                        acc[4 * q + 1] += w00 * v00.y + w10 * v10.y + w01 * v01.y + w11 * v11.y;
-                        acc[4 * q + 2] += w00 * v00.z + w10 * v10.z + w01 * v01.z + w11 * v11.z;
-                        acc[4 * q + 3] += w00 * v00.w + w10 * v10.w + w01 * v01.w + w11 * v11.w;
-                    }
-                }
+                const int i0 = fxq >> FB, j0 = fyq >> FB;
+                const float wx = __uint_as_float((((unsigned)fxq & fmask) << msh) | 0x3f800000u) - 1.f;
+                const float wy = __uint_as_float((((unsigned)fyq & fmask) << msh) | 0x3f800000u) - 1.f;
+                const int off = j0 * rowstride + i0 * Tp;
+                const float4 *p00 = reinterpret_cast<const float4 *>(slice + off);
+                const float4 *p01 = reinterpret_cast<const float4 *>(slice + (off + rowstride));
+                const float w11 = wx * wy, w10 = wx - w11, w01 = wy - w11, w00 = (1.f - wx) - w01;
+                const float4 v00 = __ldg(p00), v10 = __ldg(p00 + FG), v01 = __ldg(p01), v11 = __ldg(p01 + FG);
+                acc[0] = fmaf(w11, v11.x, fmaf(w01, v01.x, fmaf(w10, v10.x, fmaf(w00, v00.x, acc[0]))));
+                acc[1] = fmaf(w11, v11.y, fmaf(w01, v01.y, fmaf(w10, v10.y, fmaf(w00, v00.y, acc[1]))));
+                acc[2] = fmaf(w11, v11.z, fmaf(w01, v01.z, fmaf(w10, v10.z, fmaf(w00, v00.z, acc[2]))));
+                acc[3] = fmaf(w11, v11.w, fmaf(w01, v01.w, fmaf(w10, v10.w, fmaf(w00, v00.w, acc[3]))));
+                fxq += dxq;
+                fyq += dyq;
             }
         }
     }
 
     // combine the KSPLIT partial sums of a ray (fixed order: deterministic)
     if (p.KSPLIT > 1) {
-        const int nbf = p.BINS * p.FG;
-        const int idx = bl * p.FG + fg;
+        const int nbf = p.BINS * FG;
+        const int idx = bl * FG + fg;
         if (kc > 0) {
 #pragma unroll
             for (int f = 0; f < FPT; ++f) red[((kc - 1) * FPT + f) * nbf + idx] = acc[f];
@@ -195,7 +208,7 @@ __global__ void __launch_bounds__(256) k_forward(KGeom g, FwdArgs p) {
     }
     if (kc != 0 || b >= g.B) return;
 
-    const size_t o = (((size_t)z * p.As + la) * g.B + b) * p.Tp + fg * FPT;
+    const size_t o = (((size_t)z * p.As + la) * g.B + b) * Tp + fg * FPT;
     if (!p.ratio) {
 #pragma unroll
         for (int q = 0; q < FPT / 4; ++q)
@@ -203,7 +216,7 @@ __global__ void __launch_bounds__(256) k_forward(KGeom g, FwdArgs p) {
                                                                   g.step_mm * acc[4 * q + 2], g.step_mm * acc[4 * q + 3]);
     } else {
         // O1: yhat = scale A_s x + r ; q = y / yhat where yhat > 1e-12 else 0
-        const size_t oy = (((size_t)z * g.A + a) * g.B + b) * p.Tp + fg * FPT;
+        const size_t oy = (((size_t)z * g.A + a) * g.B + b) * Tp + fg * FPT;
         const float sc = p.scale * g.step_mm;
 #pragma unroll
         for (int q = 0; q < FPT / 4; ++q) {
@@ -234,6 +247,11 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
     p.As = subset < 0 ? g.A : g.A / g.S;
     p.subset = subset;
     p.ratio = ratio; p.r_mode = r_mode; p.scale = scale;
+    {   // fractional bits of the fixed-point sample coordinates: 1 sign + ceil(log2(max dim + 32)) integer bits
+        int ib = 1;
+        while ((1 << ib) < (g.nxp > g.nyp ? g.nxp : g.nyp) + 2 * KCS_ANCHOR) ++ib;
+        p.FB = 31 - ib > 22 ? 22 : 31 - ib;
+    }
     // parallelism: split the K steps of a ray over KSPLIT threads when there are too few rays to fill 148 SMs
     const long long base = (long long)g.nz * p.As * g.B * p.FG;
     int ks = 1;
@@ -248,10 +266,11 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
     const size_t smem = ks > 1 ? (size_t)(ks - 1) * FPT * bins * p.FG * sizeof(float) : 0;
     dim3 grid((g.B + bins - 1) / bins, p.As, g.nz);
     ProfScope ps(c, KCS_K_FORWARD);
-    switch (FPT) {
+    switch (p.FG) {
+        case 1: k_forward<1><<<grid, threads, smem, c->stream>>>(g, p); break;
+        case 2: k_forward<2><<<grid, threads, smem, c->stream>>>(g, p); break;
         case 4: k_forward<4><<<grid, threads, smem, c->stream>>>(g, p); break;
-        case 8: k_forward<8><<<grid, threads, smem, c->stream>>>(g, p); break;
-        default: k_forward<12><<<grid, threads, smem, c->stream>>>(g, p); break;
+        default: k_forward<8><<<grid, threads, smem, c->stream>>>(g, p); break;
     }
     LAUNCH_CHECK(c);
     return KCS_OK;
@@ -299,6 +318,14 @@ __device__ __forceinline__ float4 voxel_angle_weights(const KGeom &g, int a, int
     return make_float4(__int_as_float(b0c), wo[0], wo[1], wo[2]);
 }
 
+// O2 / eq. 2-3 with Q7-Q10, one division:  x bp / max(S (1 + beta (x-F)/Fm), 0.1 S)  with Fm = max(F, 1e-20)
+//   = x bp Fm / (S max(Fm + beta (x-F), 0.1 Fm)).
+__device__ __forceinline__ float osl_one(float x, float bp, float F, float S, float beta) {
+    const float Fm = fmaxf(F, 1e-20f);
+    const float den = S * fmaxf(fmaf(beta, x - F, Fm), 0.1f * Fm);
+    return __fdividef(x * bp * Fm, den);
+}
+
 struct BackArgs {
     const float *qi;
     float *out;          // padded inner layout (plain back-projection) or xi (OSL, in place)
@@ -306,61 +333,123 @@ struct BackArgs {
     const float *sens;   // [ny][nx] unscaled A_s^T 1 of this subset
     const float *smax;   // device scalar: max(sens)
     const unsigned char *mask;
-    int Tp, FG, TX, TY, As, subset, osl;
+    const float4 *wtab;  // [A][nbj][nbi4][KCS_BW][4] block-angle weight records (k_build_wtab)
+    int nbj, nbi4;
+    int Tp, FG, BX, BY, As, subset, osl;  // BX x BY blocks of 2x2 voxels per CTA
     float scale, beta;
 };
 
-#define KCS_BACK_ACH 16  // angles per shared-memory weight chunk
+#define KCS_BW 6  // float4 per (block, angle) weight record: {base bin, w[4 voxels][5 bins], pad}
 
-template <int FPT, int ZB>
+// Geometry-only table, built once per context: for every angle a and every 2x2 voxel block (bi, bj) the base bin of the
+// block's 5-bin window and the 4 x 5 tent weights (zero where a voxel does not see a bin; P4 / SURVEY H2).  Records of
+// 4 x-adjacent blocks are interleaved float4-wise so that a warp's request for record word r is one 64 B run.
+__global__ void k_build_wtab(KGeom g, float4 *wtab, int nbi, int nbj, int nbi4) {
+    const int bi = blockIdx.x * blockDim.x + threadIdx.x;
+    const int bj = blockIdx.y, a = blockIdx.z;
+    if (bi >= nbi4 * 4) return;
+    float4 w4[4];
+    int bmin = 1 << 30;
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+        const int vi = 2 * bi + (v & 1), vj = 2 * bj + (v >> 1);
+        if (bi < nbi && vi < g.nx && vj < g.ny) {
+            w4[v] = voxel_angle_weights(g, a, vi, vj);  // {b0c, w0, w1, w2}, b0c in [0, B-3]
+            bmin = min(bmin, __float_as_int(w4[v].x));
+        } else {
+            w4[v] = make_float4(__int_as_float(1 << 30), 0.f, 0.f, 0.f);
+        }
+    }
+    const int base = max(0, min(bmin, g.B - 5));
+    float w[4][5];
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+        const int sh = __float_as_int(w4[v].x) - base;  // 0..2 for an in-image voxel
+#pragma unroll
+        for (int r = 0; r < 5; ++r) {
+            const int q = r - sh;
+            w[v][r] = (q == 0) ? w4[v].y : (q == 1) ? w4[v].z : (q == 2) ? w4[v].w : 0.f;
+        }
+    }
+    float4 *rec = wtab + (((size_t)a * nbj + bj) * nbi4 + (bi >> 2)) * (KCS_BW * 4) + (bi & 3);
+    rec[0] = make_float4(__int_as_float(base), w[0][0], w[0][1], w[0][2]);
+    rec[4] = make_float4(w[0][3], w[0][4], w[1][0], w[1][1]);
+    rec[8] = make_float4(w[1][2], w[1][3], w[1][4], w[2][0]);
+    rec[12] = make_float4(w[2][1], w[2][2], w[2][3], w[2][4]);
+    rec[16] = make_float4(w[3][0], w[3][1], w[3][2], w[3][3]);
+    rec[20] = make_float4(w[3][4], 0.f, 0.f, 0.f);
+}
+
+int kcs_launch_build_wtab(kcs_ctx *c) {
+    const KGeom &g = c->g;
+    dim3 grid((c->nbi4 * 4 + 63) / 64, c->nbj, g.A);
+    ProfScope ps(c, KCS_K_OTHER);
+    k_build_wtab<<<grid, 64, 0, c->stream>>>(g, c->d_wtab, c->nbi, c->nbj, c->nbi4);
+    LAUNCH_CHECK(c);
+    return KCS_OK;
+}
+
+// One thread = one 2x2 voxel block x 4 frames x ZB slices.  The four voxels of a block see bins inside one window of
+// 5 consecutive bins (kcs_create guarantees (|cos| vx + |sin| vy)/bin <= 1.5, so their centre bins differ by <= 2):
+// the window's 5 sinogram values are loaded once (5 LDG.128, one 128 B line each at Tp = 32) and serve all four
+// voxels: 1.25 L1 wavefronts per voxel-angle instead of 3.  Weights come from the k_build_wtab table (L2 resident:
+// it is the same for every slice and frame).  No atomics: run-to-run deterministic.
+template <int ZB>
 __global__ void __launch_bounds__(256) k_back(KGeom g, BackArgs p) {
-    extern __shared__ float4 wts[];  // [KCS_BACK_ACH][NVOX]
     const int tid = threadIdx.x;
-    const int nvox = p.TX * p.TY;
     const int fg = tid % p.FG;
-    const int vox = tid / p.FG;
-    const int i = blockIdx.x * p.TX + vox % p.TX;
-    const int j = blockIdx.y * p.TY + vox / p.TX;
+    const int blk = tid / p.FG;
+    const int bi = blockIdx.x * p.BX + blk % p.BX, bj = blockIdx.y * p.BY + blk / p.BX;
+    const int i0 = bi * 2, j0 = bj * 2;
     const int z0 = blockIdx.z * ZB;
-    const bool inimg = (vox < nvox) && (i < g.nx) && (j < g.ny);
-    bool active = inimg;
-    if (p.osl && inimg) active = p.mask[j * g.nx + i] != 0;
+    const bool inimg = (i0 < g.nx) && (j0 < g.ny);
+    bool vin[4], vact[4], active = false;
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+        const int i = i0 + (v & 1), j = j0 + (v >> 1);
+        vin[v] = (i < g.nx) && (j < g.ny);
+        vact[v] = vin[v] && (!p.osl || p.mask[j * g.nx + i] != 0);
+        active = active || vact[v];
+    }
 
-    float acc[ZB][FPT];
+    float acc[ZB][4][4];
 #pragma unroll
     for (int zb = 0; zb < ZB; ++zb)
 #pragma unroll
-        for (int f = 0; f < FPT; ++f) acc[zb][f] = 0.f;
+        for (int v = 0; v < 4; ++v)
+#pragma unroll
+            for (int f = 0; f < 4; ++f) acc[zb][v][f] = 0.f;
 
     const int Tp = p.Tp;
-    for (int la0 = 0; la0 < p.As; la0 += KCS_BACK_ACH) {
-        const int nla = min(KCS_BACK_ACH, p.As - la0);
-        __syncthreads();
-        for (int item = tid; item < nla * nvox; item += blockDim.x) {
-            const int l = item / nvox, v = item - l * nvox;
-            const int vi = blockIdx.x * p.TX + v % p.TX, vj = blockIdx.y * p.TY + v / p.TX;
-            const int a = p.subset < 0 ? (la0 + l) : p.subset + (la0 + l) * g.S;
-            wts[item] = voxel_angle_weights(g, a, vi, vj);
-        }
-        __syncthreads();
-        if (active) {
-            for (int l = 0; l < nla; ++l) {
-                const float4 w = wts[l * nvox + vox];
-                const int b0 = __float_as_int(w.x);
+    if (active) {
+        const size_t astride = (size_t)p.nbj * p.nbi4 * (KCS_BW * 4);
+        const float4 *rec0 = p.wtab + ((size_t)bj * p.nbi4 + (bi >> 2)) * (KCS_BW * 4) + (bi & 3);
+        for (int l = 0; l < p.As; ++l) {
+            const int a = p.subset < 0 ? l : p.subset + l * g.S;
+            const float4 *rec = rec0 + (size_t)a * astride;
+            const float4 r0 = __ldg(rec), r1 = __ldg(rec + 4), r2 = __ldg(rec + 8), r3 = __ldg(rec + 12),
+                         r4 = __ldg(rec + 16), r5 = __ldg(rec + 20);
+            const int base = __float_as_int(r0.x);
+            const float w[4][5] = {{r0.y, r0.z, r0.w, r1.x, r1.y},
+                                   {r1.z, r1.w, r2.x, r2.y, r2.z},
+                                   {r2.w, r3.x, r3.y, r3.z, r3.w},
+                                   {r4.x, r4.y, r4.z, r4.w, r5.x}};
 #pragma unroll
-                for (int zb = 0; zb < ZB; ++zb) {
-                    const int z = z0 + zb;
-                    if (z < g.nz) {
-                        const float *row = p.qi + (((size_t)z * p.As + (la0 + l)) * g.B + b0) * Tp + fg * FPT;
+            for (int zb = 0; zb < ZB; ++zb) {
+                const int z = z0 + zb;
+                if (z < g.nz) {
+                    const float *row = p.qi + (((size_t)z * p.As + l) * g.B + base) * Tp + fg * 4;
+                    float4 q[5];
 #pragma unroll
-                        for (int q = 0; q < FPT / 4; ++q) {
-                            const float4 q0 = __ldg(reinterpret_cast<const float4 *>(row) + q);
-                            const float4 q1 = __ldg(reinterpret_cast<const float4 *>(row + Tp) + q);
-                            const float4 q2 = __ldg(reinterpret_cast<const float4 *>(row + 2 * Tp) + q);
-                            acc[zb][4 * q + 0] += w.y * q0.x + w.z * q1.x + w.w * q2.x;
-                            acc[zb][4 * q + 1] += w.y * q0.y + w.z * q1.y + w.w * q2.y;
-                            acc[zb][4 * q + 2] += w.y * q0.z + w.z * q1.z + w.w * q2.z;
-                            acc[zb][4 * q + 3] += w.y * q0.w + w.z * q1.w + w.w * q2.w;
+                    for (int r = 0; r < 5; ++r) q[r] = __ldg(reinterpret_cast<const float4 *>(row + r * Tp));
+#pragma unroll
+                    for (int v = 0; v < 4; ++v) {
+#pragma unroll
+                        for (int r = 0; r < 5; ++r) {
+                            acc[zb][v][0] = fmaf(w[v][r], q[r].x, acc[zb][v][0]);
+                            acc[zb][v][1] = fmaf(w[v][r], q[r].y, acc[zb][v][1]);
+                            acc[zb][v][2] = fmaf(w[v][r], q[r].z, acc[zb][v][2]);
+                            acc[zb][v][3] = fmaf(w[v][r], q[r].w, acc[zb][v][3]);
                         }
                     }
                 }
@@ -369,60 +458,38 @@ __global__ void __launch_bounds__(256) k_back(KGeom g, BackArgs p) {
     }
     if (!inimg) return;
 
-    const float S0 = p.osl ? p.sens[j * g.nx + i] : 0.f;
     const float smax = p.osl ? *p.smax : 0.f;
+    const float sc = p.scale * g.step_mm;
 #pragma unroll
-    for (int zb = 0; zb < ZB; ++zb) {
-        const int z = z0 + zb;
-        if (z >= g.nz) break;
-        const size_t o = (((size_t)z * g.nyp + (j + 1)) * g.nxp + (i + 1)) * Tp + fg * FPT;
-        if (!p.osl) {
+    for (int v = 0; v < 4; ++v) {
+        if (!vin[v]) continue;
+        const int i = i0 + (v & 1), j = j0 + (v >> 1);
+        const float S0 = p.osl ? p.sens[j * g.nx + i] : 0.f;
+        const float S = p.scale * S0;
+        const bool dead = (!vact[v]) || !(S0 > 1e-12f * smax);
 #pragma unroll
-            for (int q = 0; q < FPT / 4; ++q)
-                reinterpret_cast<float4 *>(p.out + o)[q] =
-                    make_float4(g.step_mm * acc[zb][4 * q], g.step_mm * acc[zb][4 * q + 1],
-                                g.step_mm * acc[zb][4 * q + 2], g.step_mm * acc[zb][4 * q + 3]);
-        } else {
-            // O2 / eq. 2-3 with Q7-Q10:  x <- x * bp / max(S (1 + beta (x-F)/max(F,1e-20)), 0.1 S)
-            const float S = p.scale * S0;
-            const bool dead = (!active) || !(S0 > 1e-12f * smax);
-            const float sc = p.scale * g.step_mm;
-#pragma unroll
-            for (int q = 0; q < FPT / 4; ++q) {
-                float4 xv = reinterpret_cast<const float4 *>(p.out + o)[q];
+        for (int zb = 0; zb < ZB; ++zb) {
+            const int z = z0 + zb;
+            if (z >= g.nz) break;
+            const size_t o = (((size_t)z * g.nyp + (j + KCS_PAD)) * g.nxp + (i + KCS_PAD)) * Tp + fg * 4;
+            if (!p.osl) {
+                *reinterpret_cast<float4 *>(p.out + o) = make_float4(g.step_mm * acc[zb][v][0], g.step_mm * acc[zb][v][1],
+                                                                     g.step_mm * acc[zb][v][2], g.step_mm * acc[zb][v][3]);
+            } else {
+                // O2 / eq. 2-3 with Q7-Q10:  x <- x * bp / max(S (1 + beta (x-F)/max(F,1e-20)), 0.1 S)
+                float4 xv = *reinterpret_cast<const float4 *>(p.out + o);
                 if (dead) {
                     xv = make_float4(0.f, 0.f, 0.f, 0.f);
                 } else {
-                    const float4 Fv = __ldg(reinterpret_cast<const float4 *>(p.Fi + o) + q);
-                    float D;
-                    D = S * (1.f + p.beta * (xv.x - Fv.x) / fmaxf(Fv.x, 1e-20f)); D = fmaxf(D, 0.1f * S);
-                    xv.x = xv.x * (sc * acc[zb][4 * q + 0]) / D;
-                    D = S * (1.f + p.beta * (xv.y - Fv.y) / fmaxf(Fv.y, 1e-20f)); D = fmaxf(D, 0.1f * S);
-                    xv.y = xv.y * (sc * acc[zb][4 * q + 1]) / D;
-                    D = S * (1.f + p.beta * (xv.z - Fv.z) / fmaxf(Fv.z, 1e-20f)); D = fmaxf(D, 0.1f * S);
-                    xv.z = xv.z * (sc * acc[zb][4 * q + 2]) / D;
-                    D = S * (1.f + p.beta * (xv.w - Fv.w) / fmaxf(Fv.w, 1e-20f)); D = fmaxf(D, 0.1f * S);
-                    xv.w = xv.w * (sc * acc[zb][4 * q + 3]) / D;
+                    const float4 Fv = __ldg(reinterpret_cast<const float4 *>(p.Fi + o));
+                    xv.x = osl_one(xv.x, sc * acc[zb][v][0], Fv.x, S, p.beta);
+                    xv.y = osl_one(xv.y, sc * acc[zb][v][1], Fv.y, S, p.beta);
+                    xv.z = osl_one(xv.z, sc * acc[zb][v][2], Fv.z, S, p.beta);
+                    xv.w = osl_one(xv.w, sc * acc[zb][v][3], Fv.w, S, p.beta);
                 }
-                reinterpret_cast<float4 *>(p.out + o)[q] = xv;
+                *reinterpret_cast<float4 *>(p.out + o) = xv;
             }
         }
-    }
-}
-
-template <int FPT>
-static void back_dispatch(int ZB, dim3 grid, int threads, size_t smem, cudaStream_t st, const KGeom &g, const BackArgs &p) {
-    static bool optin = false;  // the weight chunk can exceed the 48 KB default (64 KB at 256 voxels per block)
-    if (!optin) {
-        cudaFuncSetAttribute(k_back<FPT, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
-        cudaFuncSetAttribute(k_back<FPT, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
-        cudaFuncSetAttribute(k_back<FPT, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
-        optin = true;
-    }
-    switch (ZB) {
-        case 4: k_back<FPT, 4><<<grid, threads, smem, st>>>(g, p); break;
-        case 2: k_back<FPT, 2><<<grid, threads, smem, st>>>(g, p); break;
-        default: k_back<FPT, 1><<<grid, threads, smem, st>>>(g, p); break;
     }
 }
 
@@ -437,28 +504,25 @@ int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, f
     p.smax = c->d_smax + sidx;
     p.mask = c->d_mask;
     p.Tp = Tp;
-    const int FPT = choose_fpt(Tp);
-    p.FG = Tp / FPT;
+    p.FG = Tp / 4;
     p.As = subset < 0 ? g.A : g.A / g.S;
     p.subset = subset;
     p.osl = osl; p.scale = scale; p.beta = beta;
-    const int nv = 256 / p.FG;
-    p.TX = nv >= 128 ? 32 : (nv >= 64 ? 16 : 8);
-    p.TY = nv / p.TX;
-    const int nvox = p.TX * p.TY;
-    const int threads = nvox * p.FG;
-    const int gx = (g.nx + p.TX - 1) / p.TX, gy = (g.ny + p.TY - 1) / p.TY;
+    p.wtab = c->d_wtab; p.nbj = c->nbj; p.nbi4 = c->nbi4;
+    const int nblk = 256 / p.FG;                 // 32 .. 256 voxel blocks per CTA
+    p.BX = nblk >= 128 ? 16 : 8;
+    p.BY = nblk / p.BX;
+    const int gx = (g.nx + 2 * p.BX - 1) / (2 * p.BX), gy = (g.ny + 2 * p.BY - 1) / (2 * p.BY);
     int ZB = 1;
-    if (g.nz >= 4 && (long long)gx * gy * ((g.nz + 3) / 4) >= 148LL * 8) ZB = 4;
-    else if (g.nz >= 2 && (long long)gx * gy * ((g.nz + 1) / 2) >= 148LL * 8) ZB = 2;
-    if (FPT == 12 && ZB == 4) ZB = 2;  // register budget
+    if (g.nz >= 4 && (long long)gx * gy * ((g.nz + 3) / 4) >= 148LL * 4) ZB = 4;
+    else if (g.nz >= 2 && (long long)gx * gy * ((g.nz + 1) / 2) >= 148LL * 4) ZB = 2;
+    if (const char *e = getenv("KCS_ZB")) ZB = atoi(e);
     dim3 grid(gx, gy, (g.nz + ZB - 1) / ZB);
-    const size_t smem = (size_t)KCS_BACK_ACH * nvox * sizeof(float4);
     ProfScope ps(c, KCS_K_BACK);
-    switch (FPT) {
-        case 4: back_dispatch<4>(ZB, grid, threads, smem, c->stream, g, p); break;
-        case 8: back_dispatch<8>(ZB, grid, threads, smem, c->stream, g, p); break;
-        default: back_dispatch<12>(ZB, grid, threads, smem, c->stream, g, p); break;
+    switch (ZB) {
+        case 4: k_back<4><<<grid, 256, 0, c->stream>>>(g, p); break;
+        case 2: k_back<2><<<grid, 256, 0, c->stream>>>(g, p); break;
+        default: k_back<1><<<grid, 256, 0, c->stream>>>(g, p); break;
     }
     LAUNCH_CHECK(c);
     return KCS_OK;
