@@ -142,6 +142,21 @@ def dist_env():
     return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
 
 
+def max_over_ranks(seconds: float, dist, device) -> float:
+    """Replicas only: the job's time is the slowest rank's; no collective touches the data path."""
+    if dist is None:
+        return seconds
+    import torch
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_throughput(world: int, steps: int, seconds: float) -> float:
+    """Whole-job ICM iterations/s of `world` independent replicas that each ran `steps` iterations in `seconds` (max)."""
+    return world * steps / seconds
+
+
 def load_traffic(workload: str, cls: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
     `ncu --set full` capture (profiles/traffic.csv: workload,kernel_class,dram_bytes_per_launch), or None."""
@@ -221,12 +236,9 @@ def run_ours(args):
     barrier()
     launches = ctx.launch_count() - n0
     ms_total = float(sum(a.elapsed_time(b) for a, b in evs))
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dist, dev)
     ms_per_step = ms_total / args.steps
-    value = world * args.steps / (ms_total * 1e-3)
+    value = replica_throughput(world, args.steps, ms_total * 1e-3)
 
     # ---- per-kernel pass (same steps again, profiling events on) -> roofline of the dominant kernel
     ctx.profile_enable(True)
@@ -310,13 +322,10 @@ def run_e2e(ctx, cfg, prob, state0, torch, args, world, dist, dev, flush):
     if dist is not None:
         dist.barrier()
     tot = sum(one(i) for i in range(args.steps))
-    if dist is not None:
-        t = torch.tensor([tot], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        tot = float(t.item())
+    tot = max_over_ranks(tot, dist, dev)
     h2d = 4 * (hy.numel() + hr.numel() + hx.numel() + hth.numel() + hlam.numel())
     d2h = 4 * (hx.numel() + hth.numel() + hlam.numel())
-    return {"value": world * args.steps / tot, "unit": UNIT, "ms_per_step": 1e3 * tot / args.steps,
+    return {"value": replica_throughput(world, args.steps, tot), "unit": UNIT, "ms_per_step": 1e3 * tot / args.steps,
             "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
             "api": "kcs_icm_run_host (n_iter = 1), pinned host buffers, wall clock around the synchronous call"}
 
