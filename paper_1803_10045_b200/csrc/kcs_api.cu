@@ -242,7 +242,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     KGeom &g = c->g;
     g.nx = nx; g.ny = ny; g.nz = nz; g.nxp = nx + 2 * KCS_PAD; g.nyp = ny + 2 * KCS_PAD;
     g.A = A; g.B = B; g.K = K; g.S = cfg->n_subsets;
-    g.step_mm = cfg->step_mm;
+    g.step_mm = cfg->step_mm; g.bin_mm = cfg->bin_mm;
     g.cx = 0.5 * (nx - 1); g.cy = 0.5 * (ny - 1); g.cb = 0.5 * (B - 1); g.ck = 0.5 * (K - 1);
     c->n_vox = (size_t)nz * ny * nx;
     c->n_pix_pad = (size_t)nz * g.nyp * g.nxp;
@@ -270,6 +270,17 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
                 const double X = (i - g.cx) * cfg->vx, Y = (j - g.cy) * cfg->vy;
                 c->h_mask[(size_t)j * nx + i] = (X * X + Y * Y <= rad * rad) ? 1 : 0;
             }
+    }
+    {   // radius of the smallest centred circle that holds every in-mask voxel centre, plus 1.5 voxels for the taps
+        double r2 = 0.0;
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i)
+                if (c->h_mask[(size_t)j * nx + i]) {
+                    const double X = (i - g.cx) * cfg->vx, Y = (j - g.cy) * cfg->vy;
+                    if (X * X + Y * Y > r2) r2 = X * X + Y * Y;
+                }
+        const double rc = std::sqrt(r2) + 1.5 * (cfg->vx > cfg->vy ? cfg->vx : cfg->vy);
+        c->fov_rc2 = (float)(rc * rc);
     }
     // K1, K3, K4: kinetic tables (fp64 via long-double quadrature)
     Feng fe;
@@ -362,7 +373,7 @@ int kcs_forward_project(kcs_ctx *c, const float *x, float *y_s, int subset, int 
     const int Tp = round_up4(nf), As = subset < 0 ? g.A : g.A / g.S;
     if ((rc = ensure_border(c, Tp))) return rc;
     if ((rc = pack_image(c, x + (size_t)f0 * c->n_vox, nf, c->xi, Tp))) return rc;
-    if ((rc = kcs_launch_forward(c, Tp, subset, 0, 1.f, 0))) return rc;
+    if ((rc = kcs_launch_forward(c, Tp, subset, 0, 1.f, 0, 0))) return rc;
     return unpack_sino(c, c->qi, Tp, y_s + (size_t)f0 * g.nz * As * g.B, nf, As);
 }
 
@@ -455,7 +466,8 @@ int kcs_icm_run(kcs_ctx *c, const float *y, const float *r, int r_mode, float sc
         // F <- K(theta^{n-1}), held fixed during the pass ("one step late")
         if ((rc = kcs_launch_kinetic(c, theta, c->Fi, nullptr, 1, Tp))) return rc;
         for (int s = 0; s < g.S; ++s) {  // Q5: subsets in order 0..S-1
-            if ((rc = kcs_launch_forward(c, Tp, s, 1, scale, r_mode))) return rc;
+            // after the first OSL update of this call x is zero outside the mask: rays are clipped to the FOV circle
+            if ((rc = kcs_launch_forward(c, Tp, s, 1, scale, r_mode, (it > 0 || s > 0) ? 1 : 0))) return rc;
             if ((rc = kcs_launch_back(c, Tp, s, 1, nullptr, scale, b))) return rc;
         }
         if ((rc = lm_steps(c, c->xi, 1, Tp, theta, lambda, gamma, delta, n_lm, nullptr))) return rc;

@@ -21,7 +21,7 @@ struct KGeom {
     int nx, ny, nz;
     int nxp, nyp;      // nx + 2 KCS_PAD, ny + 2 KCS_PAD
     int A, B, K, S;
-    float step_mm;
+    float step_mm, bin_mm;
     double cx, cy, cb, ck;  // (nx-1)/2, (ny-1)/2, (B-1)/2, (K-1)/2
     // per-angle tables (device, double4 each):
     //   fwd[a] = (bin cos/vx, -step sin/vx, bin sin/vy, step cos/vy):  fx = (b-cb) f.x + (k-ck) f.y + cx ; fy = (b-cb) f.z + (k-ck) f.w + cy
@@ -97,6 +97,7 @@ struct kcs_ctx {
     float *r_pad;  // [32] per-frame randoms padded with 0
     float *theta2;  // [4][n_vox] ping-pong buffer for the Jacobi LM steps
     int xi_border_tp;  // Tp for which xi's zero border is valid (0 = unknown)
+    float fov_rc2;     // (mask radius + 1.5 voxels)^2, mm^2: rays are clipped to this circle when x is known to be masked
 
     // device staging buffers of kcs_icm_run_host, allocated lazily
     float *st_y, *st_r, *st_x, *st_theta, *st_lambda;
@@ -160,7 +161,7 @@ int kcs_launch_unpack(kcs_ctx *c, const float *src, int Tp, float *dst, size_t f
 // forward projection of c->xi (Tp frames) for `subset`; out = c->qi.
 //   ratio == 0:  qi = step * sum                      (kcs_forward_project)
 //   ratio == 1:  qi = y / (scale*step*sum + r), 0 where the denominator <= 1e-12   (O1)
-int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, int r_mode);
+int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, int r_mode, int clip_fov);
 // gather back-projection of c->qi for `subset`.
 //   osl == 0:  out_inner (padded layout) = step * sum                              (kcs_back_project)
 //   osl == 1:  c->xi <- OSL update with bp = scale*step*sum, sens = scale*A_s^T 1, F = c->Fi   (O2)

@@ -117,14 +117,29 @@ struct FwdArgs {
     int As, subset;
     int ratio, r_mode;
     float scale;
+    float clip_r2;       // >= 0: x is zero outside a centred circle of this squared radius (mm^2)
 };
 
 #define KCS_ANCHOR 16  // steps between fp64 re-anchoring of the sample coordinates
+#ifndef KCS_FWD_UNROLL
+#define KCS_FWD_UNROLL 4
+#endif
+#ifndef KCS_FWD_MINBLK
+#define KCS_FWD_MINBLK 1
+#endif
+#ifndef KCS_FWD_TPB
+#define KCS_FWD_TPB 128
+#endif
+#ifndef KCS_BACK_MINBLK
+#define KCS_BACK_MINBLK 1
+#endif
+#define KCS_STR2(x) #x
+#define KCS_STR(x) KCS_STR2(x)
 
 // One thread = one ray x 4 frames; the FG = Tp/4 lanes of a ray read a whole pixel (16 FG bytes) per tap in one request.
 template <int FG>
-__global__ void __launch_bounds__(256) k_forward(KGeom g, FwdArgs p) {
-    constexpr int FPT = 4, Tp = 4 * FG;
+__global__ void __launch_bounds__(KCS_FWD_TPB, KCS_FWD_MINBLK) k_forward(KGeom g, FwdArgs p) {
+    constexpr int FPT = 4, Tp = 4 * FG, kUnroll = KCS_FWD_UNROLL;
     extern __shared__ float red[];
     const int tid = threadIdx.x;
     const int fg = tid % FG;
@@ -162,6 +177,11 @@ __global__ void __launch_bounds__(256) k_forward(KGeom g, FwdArgs p) {
             if (fabs(fw.w) < 1e-9) { if (!(pya >= lo && pya < hy)) thi = -1.0; }
             else { const double t0 = (lo - pya) / fw.w, t1 = (hy - pya) / fw.w; tlo = fmax(tlo, fmin(t0, t1) + 1e-6); thi = fmin(thi, fmax(t0, t1) - 1e-6); }
         }
+        if (p.clip_r2 >= 0.f) {  // samples farther than the mask radius + 1.5 voxels from the axis only see zeros
+            const double sb = bc * (double)g.bin_mm, h2 = (double)p.clip_r2 - sb * sb;
+            if (h2 < 0.0) thi = -1.0;
+            else { const double h = sqrt(h2) / (double)g.step_mm; tlo = fmax(tlo, g.ck - h); thi = fmin(thi, g.ck + h); }
+        }
         const int k_lo = (int)ceil(tlo);       // clip bounds were moved 1e-6 steps inwards: strictly inside the margin
         const int k_hi = (int)floor(thi) + 1;
         const int rowstride = g.nxp * Tp;
@@ -171,7 +191,7 @@ __global__ void __launch_bounds__(256) k_forward(KGeom g, FwdArgs p) {
             const double kk = (double)k0;
             int fxq = __double2int_rn(fma(kk, fw.y, pxa) * qs), fyq = __double2int_rn(fma(kk, fw.w, pya) * qs);
             const int mmax = min(KCS_ANCHOR, k_hi - k0);
-#pragma unroll 4
+#pragma unroll(kUnroll)
             for (int m = 0; m < mmax; ++m) {
                 const int i0 = fxq >> FB, j0 = fyq >> FB;
                 const float wx = __uint_as_float((((unsigned)fxq & fmask) << msh) | 0x3f800000u) - 1.f;
@@ -237,7 +257,7 @@ __global__ void __launch_bounds__(256) k_forward(KGeom g, FwdArgs p) {
     }
 }
 
-int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, int r_mode) {
+int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, int r_mode, int clip_fov) {
     const KGeom &g = c->g;
     FwdArgs p;
     p.xi = c->xi; p.qi = c->qi; p.yi = c->yi; p.ri = c->ri; p.r_pad = c->r_pad;
@@ -247,6 +267,7 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
     p.As = subset < 0 ? g.A : g.A / g.S;
     p.subset = subset;
     p.ratio = ratio; p.r_mode = r_mode; p.scale = scale;
+    p.clip_r2 = clip_fov ? c->fov_rc2 : -1.f;
     {   // fractional bits of the fixed-point sample coordinates: 1 sign + ceil(log2(max dim + 32)) integer bits
         int ib = 1;
         while ((1 << ib) < (g.nxp > g.nyp ? g.nxp : g.nyp) + 2 * KCS_ANCHOR) ++ib;
@@ -258,7 +279,7 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
     while (base * ks < 148LL * 2048 && ks < 8 && g.K / (ks * 2) >= 16) ks *= 2;
     p.KSPLIT = ks;
     p.KCH = (g.K + ks - 1) / ks;
-    int bins = 128 / (p.FG * ks);
+    int bins = KCS_FWD_TPB / (p.FG * ks);
     if (bins < 1) bins = 1;
     if (bins > g.B) bins = g.B;
     p.BINS = bins;
@@ -395,7 +416,7 @@ int kcs_launch_build_wtab(kcs_ctx *c) {
 // voxels: 1.25 L1 wavefronts per voxel-angle instead of 3.  Weights come from the k_build_wtab table (L2 resident:
 // it is the same for every slice and frame).  No atomics: run-to-run deterministic.
 template <int ZB>
-__global__ void __launch_bounds__(256) k_back(KGeom g, BackArgs p) {
+__global__ void __launch_bounds__(256, KCS_BACK_MINBLK) k_back(KGeom g, BackArgs p) {
     const int tid = threadIdx.x;
     const int fg = tid % p.FG;
     const int blk = tid / p.FG;
@@ -514,8 +535,8 @@ int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, f
     p.BY = nblk / p.BX;
     const int gx = (g.nx + 2 * p.BX - 1) / (2 * p.BX), gy = (g.ny + 2 * p.BY - 1) / (2 * p.BY);
     int ZB = 1;
-    if (g.nz >= 4 && (long long)gx * gy * ((g.nz + 3) / 4) >= 148LL * 4) ZB = 4;
-    else if (g.nz >= 2 && (long long)gx * gy * ((g.nz + 1) / 2) >= 148LL * 4) ZB = 2;
+    if (g.nz >= 4 && (long long)gx * gy * ((g.nz + 3) / 4) >= 148LL) ZB = 4;  // measured on C2: 256 CTAs of ZB = 4 beat 1024 of ZB = 1
+    else if (g.nz >= 2 && (long long)gx * gy * ((g.nz + 1) / 2) >= 148LL) ZB = 2;
     if (const char *e = getenv("KCS_ZB")) ZB = atoi(e);
     dim3 grid(gx, gy, (g.nz + ZB - 1) / ZB);
     ProfScope ps(c, KCS_K_BACK);
