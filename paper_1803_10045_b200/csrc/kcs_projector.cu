@@ -8,7 +8,6 @@
 // ray sample (forward) or one voxel (backward); each lane owns FPT frames as float4 registers.  Geometry math is
 // frame-independent and amortised over the FPT frames; coalescing comes from the frame axis and therefore does
 // not depend on the projection angle.
-#include <cstdlib>
 #include "kcs_internal.cuh"
 
 #define LAUNCH_CHECK(c)                                                     \
@@ -537,7 +536,6 @@ int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, f
     int ZB = 1;
     if (g.nz >= 4 && (long long)gx * gy * ((g.nz + 3) / 4) >= 148LL) ZB = 4;  // measured on C2: 256 CTAs of ZB = 4 beat 1024 of ZB = 1
     else if (g.nz >= 2 && (long long)gx * gy * ((g.nz + 1) / 2) >= 148LL) ZB = 2;
-    if (const char *e = getenv("KCS_ZB")) ZB = atoi(e);
     dim3 grid(gx, gy, (g.nz + ZB - 1) / ZB);
     ProfScope ps(c, KCS_K_BACK);
     switch (ZB) {
