@@ -441,6 +441,22 @@ __global__ void __launch_bounds__(256, KCS_BACK_MINBLK) k_back(KGeom g, BackArgs
             for (int f = 0; f < 4; ++f) acc[zb][v][f] = 0.f;
 
     const int Tp = p.Tp;
+    if (p.osl && active) {
+        // the epilogue's x and F lines come from HBM (they do not fit L2 between subsets at C4): start them now
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+            if (!vact[v]) continue;
+            const int i = i0 + (v & 1), j = j0 + (v >> 1);
+#pragma unroll
+            for (int zb = 0; zb < ZB; ++zb) {
+                const int z = z0 + zb;
+                if (z >= g.nz) break;
+                const size_t o = (((size_t)z * g.nyp + (j + KCS_PAD)) * g.nxp + (i + KCS_PAD)) * Tp + fg * 4;
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(p.out + o));
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(p.Fi + o));
+            }
+        }
+    }
     if (active) {
         const size_t astride = (size_t)p.nbj * p.nbi4 * (KCS_BW * 4);
         const float4 *rec0 = p.wtab + ((size_t)bj * p.nbi4 + (bi >> 2)) * (KCS_BW * 4) + (bi & 3);
