@@ -198,7 +198,7 @@ int kcs_destroy(kcs_ctx *c) {
     if (!c) return KCS_ERR_NULL;
     cudaStreamSynchronize(c->stream);
     void *ptrs[] = {c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->d_wtab, c->xi, c->Fi,
-                    c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
+                    c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->thD[0], c->thD[1], c->lamD, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     for (const KProfRec &r : c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -235,6 +235,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->d_sens = c->d_smax = c->d_tmp_smax = nullptr;
     c->d_wtab = nullptr;
     c->xi = c->Fi = c->qi = c->yi = c->ri = c->r_pad = c->theta2 = nullptr;
+    c->thD[0] = c->thD[1] = c->lamD = nullptr;
     c->st_y = c->st_r = c->st_x = c->st_theta = c->st_lambda = nullptr;
     c->st_r_elems = 0;
 
@@ -336,6 +337,9 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     TRY(dalloc(c, &c->yi, c->n_ray_all * Tp));
     TRY(dalloc(c, &c->r_pad, (size_t)KCS_MAX_FRAMES));
     TRY(dalloc(c, &c->theta2, 4 * c->n_vox));
+    TRY(dalloc(c, &c->thD[0], 4 * c->n_vox));
+    TRY(dalloc(c, &c->thD[1], 4 * c->n_vox));
+    TRY(dalloc(c, &c->lamD, c->n_vox));
     TRY(cudaMemcpyAsync(c->d_fwd, fw.data(), sizeof(double4) * A, cudaMemcpyHostToDevice, c->stream));
     TRY(cudaMemcpyAsync(c->d_bwd, bw.data(), sizeof(double4) * A, cudaMemcpyHostToDevice, c->stream));
     TRY(cudaMemcpyAsync(c->d_frames, frames.data(), sizeof(KFrame) * T, cudaMemcpyHostToDevice, c->stream));
@@ -416,17 +420,26 @@ int kcs_kinetic_eval(kcs_ctx *c, const float *theta, float *F, float *J) {
     return kcs_launch_kinetic(c, theta, F, J, 0, 0);
 }
 
-// n_steps Jacobi steps ping-ponging between the caller's theta and the context's second buffer.
+// n_steps Jacobi steps.  The first reads the caller's fp32 maps, the last writes them; in between the iterate lives
+// in the context's fp64 ping-pong buffers, so a call rounds theta and lambda to fp32 once, not once per step.
 static int lm_steps(kcs_ctx *c, const float *x, int x_inner, int Tp, float *theta, float *lambda, float gamma, float delta,
                     int n_steps, float *cost) {
-    float *cur = theta, *nxt = c->theta2;
-    for (int s = 0; s < n_steps; ++s) {
-        int rc = kcs_launch_lm_step(c, x, x_inner, Tp, cur, nxt, lambda, gamma, delta, (s == n_steps - 1) ? cost : nullptr);
+    if (n_steps == 1) {
+        int rc = kcs_launch_lm_step(c, x, x_inner, Tp, theta, 0, c->theta2, 0, lambda, lambda, gamma, delta, cost);
         if (rc) return rc;
-        float *t = cur; cur = nxt; nxt = t;
+        KCS_CUDA_OK(c, cudaMemcpyAsync(theta, c->theta2, 4 * c->n_vox * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+        return KCS_OK;
     }
-    if (cur != theta)
-        KCS_CUDA_OK(c, cudaMemcpyAsync(theta, cur, 4 * c->n_vox * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    for (int s = 0; s < n_steps; ++s) {
+        const bool first = s == 0, last = s == n_steps - 1;
+        const void *tin = first ? (const void *)theta : (const void *)c->thD[(s + 1) & 1];
+        void *tout = last ? (void *)theta : (void *)c->thD[s & 1];
+        const void *lin = first ? (const void *)lambda : (const void *)c->lamD;
+        void *lout = last ? (void *)lambda : (void *)c->lamD;
+        int rc = kcs_launch_lm_step(c, x, x_inner, Tp, tin, first ? 0 : 1, tout, last ? 0 : 1, lin, lout, gamma, delta,
+                                    last ? cost : nullptr);
+        if (rc) return rc;
+    }
     return KCS_OK;
 }
 

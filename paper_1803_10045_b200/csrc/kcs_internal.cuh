@@ -95,7 +95,9 @@ struct kcs_ctx {
     float *yi;   // [n_ray_all][Tp]  packed measured data
     float *ri;   // [n_ray_all][Tp]  packed randoms (KCS_R_FULL), allocated lazily
     float *r_pad;  // [32] per-frame randoms padded with 0
-    float *theta2;  // [4][n_vox] ping-pong buffer for the Jacobi LM steps
+    float *theta2;  // [4][n_vox] fp32 scratch for a single Jacobi LM step (the caller's maps cannot be updated in place)
+    double *thD[2]; // [4][n_vox] fp64 ping-pong buffers for the steps between the first and the last of a call
+    double *lamD;   // [n_vox] lambda in fp64 between those steps
     int xi_border_tp;  // Tp for which xi's zero border is valid (0 = unknown)
     float fov_rc2;     // (mask radius + 1.5 voxels)^2, mm^2: rays are clipped to this circle when x is known to be masked
 
@@ -176,5 +178,5 @@ int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *se
 int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp);
 // one Jacobi LM step: reads theta_in, writes theta_out (all voxels; masked-out voxels are copied through).
 //   x_inner == 0: x planar [T][V];  x_inner == 1: x = c->xi padded inner layout with Tp.
-int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const float *theta_in, float *theta_out,
-                       float *lambda, float gamma, float delta, float *cost);
+int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const void *theta_in, int in_f64, void *theta_out,
+                       int out_f64, const void *lam_in, void *lam_out, float gamma, float delta, float *cost);

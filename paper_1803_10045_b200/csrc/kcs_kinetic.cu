@@ -246,9 +246,13 @@ __device__ __forceinline__ bool chol4(const double m[10], const double g[4], dou
 }
 
 // 5 CTAs of 128 threads per SM (<= 102 registers): measured best of 1..8 on C2 and C4
+// TI / TO: storage type of the maps and of lambda on input / output.  Between the steps of one kcs_map_lm call the
+// iterate is kept in fp64 ping-pong buffers (TI = TO = double); only the caller's buffers are fp32.
+template <class TI, class TO>
 __global__ void __launch_bounds__(128, 5) k_lm_step(KGeom g, KKin kin, const float *__restrict__ x, int x_inner, int Tp,
-                                                 const float *__restrict__ th_in, float *__restrict__ th_out,
-                                                 float *__restrict__ lambda, const unsigned char *__restrict__ mask,
+                                                 const TI *__restrict__ th_in, TO *__restrict__ th_out,
+                                                 const TI *__restrict__ lam_in, TO *__restrict__ lam_out,
+                                                 const unsigned char *__restrict__ mask,
                                                  long long nvox, double gamma, double delta, float *cost) {
     extern __shared__ double sh_raw[];
     KFrame *fr = reinterpret_cast<KFrame *>(sh_raw);
@@ -264,7 +268,8 @@ __global__ void __launch_bounds__(128, 5) k_lm_step(KGeom g, KKin kin, const flo
     for (int p = 0; p < 4; ++p) xi[p] = th_in[(size_t)p * nvox + v];
     if (!mask[rem]) {  // out of the field of view: copied through (Q2)
 #pragma unroll
-        for (int p = 0; p < 4; ++p) th_out[(size_t)p * nvox + v] = (float)xi[p];
+        for (int p = 0; p < 4; ++p) th_out[(size_t)p * nvox + v] = (TO)xi[p];
+        lam_out[v] = (TO)lam_in[v];
         if (cost) cost[v] = 0.f;
         return;
     }
@@ -306,7 +311,7 @@ __global__ void __launch_bounds__(128, 5) k_lm_step(KGeom g, KKin kin, const flo
             gr[p] -= gamma * huber_d(t, delta);
         }
 
-    double lam = lambda[v];
+    double lam = lam_in[v];
     if (!(lam > 0.0)) lam = 1e-3 * fmax(fmax(JtJ[0], JtJ[2]), fmax(JtJ[5], JtJ[9]));  // Q15 first use
     double M[10];
 #pragma unroll
@@ -339,8 +344,8 @@ __global__ void __launch_bounds__(128, 5) k_lm_step(KGeom g, KKin kin, const flo
         }
     }
 #pragma unroll
-    for (int p = 0; p < 4; ++p) th_out[(size_t)p * nvox + v] = (float)xi[p];
-    lambda[v] = (float)lam;
+    for (int p = 0; p < 4; ++p) th_out[(size_t)p * nvox + v] = (TO)xi[p];
+    lam_out[v] = (TO)lam;
     if (cost) cost[v] = (float)phi;
 }
 
@@ -355,14 +360,22 @@ int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int i
     return KCS_OK;
 }
 
-int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const float *theta_in, float *theta_out,
-                       float *lambda, float gamma, float delta, float *cost) {
+// in_f64 / out_f64: 0 = fp32 buffers (the caller's), 1 = the context's fp64 ping-pong buffers.
+int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const void *theta_in, int in_f64, void *theta_out,
+                       int out_f64, const void *lam_in, void *lam_out, float gamma, float delta, float *cost) {
     const long long nvox = (long long)c->n_vox;
     const size_t smem = sizeof(KFrame) * c->kin.T;
+    const unsigned grid = (unsigned)((nvox + 127) / 128);
     ProfScope ps(c, KCS_K_LM);
-    k_lm_step<<<(unsigned)((nvox + 127) / 128), 128, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, theta_in, theta_out,
-                                                                        lambda, c->d_mask, nvox, (double)gamma,
-                                                                        (double)delta, cost);
+#define KCS_LM_GO(TI, TO)                                                                                              \
+    k_lm_step<TI, TO><<<grid, 128, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, (const TI *)theta_in, (TO *)theta_out, \
+                                                       (const TI *)lam_in, (TO *)lam_out, c->d_mask, nvox, (double)gamma,  \
+                                                       (double)delta, cost)
+    if (!in_f64 && !out_f64) KCS_LM_GO(float, float);
+    else if (!in_f64 && out_f64) KCS_LM_GO(float, double);
+    else if (in_f64 && out_f64) KCS_LM_GO(double, double);
+    else KCS_LM_GO(double, float);
+#undef KCS_LM_GO
     LAUNCH_CHECK(c);
     return KCS_OK;
 }
