@@ -138,7 +138,10 @@ struct FwdArgs {
 // One thread = one ray x 4 frames; the FG = Tp/4 lanes of a ray read a whole pixel (16 FG bytes) per tap in one request.
 template <int FG>
 __global__ void __launch_bounds__(KCS_FWD_TPB, KCS_FWD_MINBLK) k_forward(KGeom g, FwdArgs p) {
-    constexpr int FPT = 4, Tp = 4 * FG, kUnroll = KCS_FWD_UNROLL;
+    constexpr int FPT = 4, Tp = 4 * FG;
+    // 16 loads in flight per thread pay when a warp covers few rays (FG >= 4); with 16-32 rays per warp the extra
+    // registers cost more occupancy than the unrolling hides (C5(a) at 1 and 4 frames per launch)
+    constexpr int kUnroll = FG >= 4 ? KCS_FWD_UNROLL : 1;
     extern __shared__ float red[];
     const int tid = threadIdx.x;
     const int fg = tid % FG;
