@@ -197,7 +197,7 @@ int kcs_get_mask(const kcs_ctx *ctx, unsigned char *out) {
 int kcs_destroy(kcs_ctx *c) {
     if (!c) return KCS_ERR_NULL;
     cudaStreamSynchronize(c->stream);
-    void *ptrs[] = {c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->d_wtab, c->xi, c->Fi,
+    void *ptrs[] = {c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->d_wtab, c->d_vlist, c->xi, c->Fi,
                     c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->thD[0], c->thD[1], c->lamD, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
     for (void *p : ptrs)
         if (p) cudaFree(p);
@@ -234,6 +234,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->d_fwd = c->d_bwd = nullptr; c->d_frames = nullptr; c->d_mask = nullptr;
     c->d_sens = c->d_smax = c->d_tmp_smax = nullptr;
     c->d_wtab = nullptr;
+    c->d_vlist = nullptr; c->n_inmask2 = 0;
     c->xi = c->Fi = c->qi = c->yi = c->ri = c->r_pad = c->theta2 = nullptr;
     c->thD[0] = c->thD[1] = c->lamD = nullptr;
     c->st_y = c->st_r = c->st_x = c->st_theta = c->st_lambda = nullptr;
@@ -319,6 +320,11 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     }
     kin.beta0 = (double)fe.be[0];
 
+    std::vector<int> vlist;
+    for (int q = 0; q < nx * ny; ++q)
+        if (c->h_mask[q]) vlist.push_back(q);
+    c->n_inmask2 = (int)vlist.size();
+    vlist.resize((size_t)nx * ny, 0);
     const int Tp = round_up4(T);
     c->nbi = (nx + 1) / 2; c->nbj = (ny + 1) / 2; c->nbi4 = (c->nbi + 3) / 4;
     cudaError_t e = cudaSuccess;
@@ -327,6 +333,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     TRY(dalloc(c, &c->d_bwd, (size_t)A));
     TRY(dalloc(c, &c->d_frames, (size_t)T));
     TRY(dalloc(c, &c->d_mask, (size_t)nx * ny));
+    TRY(dalloc(c, &c->d_vlist, (size_t)nx * ny));
     TRY(dalloc(c, &c->d_sens, (size_t)(g.S + 1) * nx * ny));
     TRY(dalloc(c, &c->d_smax, (size_t)g.S + 1));
     TRY(dalloc(c, &c->d_tmp_smax, (size_t)1));
@@ -344,6 +351,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     TRY(cudaMemcpyAsync(c->d_bwd, bw.data(), sizeof(double4) * A, cudaMemcpyHostToDevice, c->stream));
     TRY(cudaMemcpyAsync(c->d_frames, frames.data(), sizeof(KFrame) * T, cudaMemcpyHostToDevice, c->stream));
     TRY(cudaMemcpyAsync(c->d_mask, c->h_mask.data(), (size_t)nx * ny, cudaMemcpyHostToDevice, c->stream));
+    TRY(cudaMemcpyAsync(c->d_vlist, vlist.data(), sizeof(int) * vlist.size(), cudaMemcpyHostToDevice, c->stream));
     TRY(cudaMemsetAsync(c->Fi, 0, c->n_pix_pad * Tp * sizeof(float), c->stream));
 #undef TRY
     if (e != cudaSuccess) {
@@ -424,10 +432,13 @@ int kcs_kinetic_eval(kcs_ctx *c, const float *theta, float *F, float *J) {
 // in the context's fp64 ping-pong buffers, so a call rounds theta and lambda to fp32 once, not once per step.
 static int lm_steps(kcs_ctx *c, const float *x, int x_inner, int Tp, float *theta, float *lambda, float gamma, float delta,
                     int n_steps, float *cost) {
-    if (n_steps == 1) {
+    const size_t map_bytes = 4 * c->n_vox * sizeof(float);
+    if (cost) KCS_CUDA_OK(c, cudaMemsetAsync(cost, 0, c->n_vox * sizeof(float), c->stream));  // out-of-mask voxels: 0
+    if (n_steps == 1) {  // fp32 scratch pre-filled with the caller's maps: the kernel only writes in-mask voxels
+        KCS_CUDA_OK(c, cudaMemcpyAsync(c->theta2, theta, map_bytes, cudaMemcpyDeviceToDevice, c->stream));
         int rc = kcs_launch_lm_step(c, x, x_inner, Tp, theta, 0, c->theta2, 0, lambda, lambda, gamma, delta, cost);
         if (rc) return rc;
-        KCS_CUDA_OK(c, cudaMemcpyAsync(theta, c->theta2, 4 * c->n_vox * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+        KCS_CUDA_OK(c, cudaMemcpyAsync(theta, c->theta2, map_bytes, cudaMemcpyDeviceToDevice, c->stream));
         return KCS_OK;
     }
     for (int s = 0; s < n_steps; ++s) {

@@ -78,6 +78,8 @@ struct kcs_ctx {
     double4 *d_fwd, *d_bwd;
     KFrame *d_frames;
     unsigned char *d_mask;            // [ny][nx]
+    int *d_vlist;                     // in-mask pixel indices j*nx+i of one slice, ascending
+    int n_inmask2;                    // their count
     std::vector<unsigned char> h_mask;
     float *d_sens;                    // [S+1][ny][nx], unscaled A_s^T 1; entry S = all angles
     float *d_smax;                    // [S+1] max over the image of d_sens[s]

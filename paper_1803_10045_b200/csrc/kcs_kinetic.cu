@@ -249,30 +249,32 @@ __device__ __forceinline__ bool chol4(const double m[10], const double g[4], dou
 // TI / TO: storage type of the maps and of lambda on input / output.  Between the steps of one kcs_map_lm call the
 // iterate is kept in fp64 ping-pong buffers (TI = TO = double); only the caller's buffers are fp32.
 template <class TI, class TO>
-__global__ void __launch_bounds__(128, 5) k_lm_step(KGeom g, KKin kin, const float *__restrict__ x, int x_inner, int Tp,
+#ifndef KCS_LM_TPB
+#define KCS_LM_TPB 128
+#endif
+#ifndef KCS_LM_MINBLK
+#define KCS_LM_MINBLK 5
+#endif
+// One thread per IN-MASK voxel: thread t of the launch fits voxel (z = t / M2, pixel vlist[t % M2]), M2 = in-mask pixels
+// of a slice.  Out-of-mask voxels get no thread (they are never read as neighbours and never written).
+__global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, KKin kin, const float *__restrict__ x, int x_inner, int Tp,
                                                  const TI *__restrict__ th_in, TO *__restrict__ th_out,
                                                  const TI *__restrict__ lam_in, TO *__restrict__ lam_out,
-                                                 const unsigned char *__restrict__ mask,
+                                                 const unsigned char *__restrict__ mask, const int *__restrict__ vlist, int M2,
                                                  long long nvox, double gamma, double delta, float *cost) {
     extern __shared__ double sh_raw[];
     KFrame *fr = reinterpret_cast<KFrame *>(sh_raw);
     load_frames(kin, fr);
-    const long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (v >= nvox) return;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)M2 * g.nz) return;
     const int v2 = g.nx * g.ny;
-    const int z = (int)(v / v2), rem = (int)(v - (long long)z * v2);
+    const int z = (int)(t / M2), rem = vlist[(int)(t - (long long)z * M2)];
+    const long long v = (long long)z * v2 + rem;
     const int j = rem / g.nx, i = rem - j * g.nx;
 
     double xi[4];
 #pragma unroll
     for (int p = 0; p < 4; ++p) xi[p] = th_in[(size_t)p * nvox + v];
-    if (!mask[rem]) {  // out of the field of view: copied through (Q2)
-#pragma unroll
-        for (int p = 0; p < 4; ++p) th_out[(size_t)p * nvox + v] = (TO)xi[p];
-        lam_out[v] = (TO)lam_in[v];
-        if (cost) cost[v] = 0.f;
-        return;
-    }
     // Q13: in-volume, in-mask 6-neighbourhood of the previous iterate (Jacobi)
     double nb[6][4];
     int nn = 0;
@@ -365,11 +367,13 @@ int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const vo
                        int out_f64, const void *lam_in, void *lam_out, float gamma, float delta, float *cost) {
     const long long nvox = (long long)c->n_vox;
     const size_t smem = sizeof(KFrame) * c->kin.T;
-    const unsigned grid = (unsigned)((nvox + 127) / 128);
+    const long long nfit = (long long)c->n_inmask2 * c->g.nz;
+    if (nfit == 0) return KCS_OK;
+    const unsigned grid = (unsigned)((nfit + KCS_LM_TPB - 1) / KCS_LM_TPB);
     ProfScope ps(c, KCS_K_LM);
 #define KCS_LM_GO(TI, TO)                                                                                              \
-    k_lm_step<TI, TO><<<grid, 128, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, (const TI *)theta_in, (TO *)theta_out, \
-                                                       (const TI *)lam_in, (TO *)lam_out, c->d_mask, nvox, (double)gamma,  \
+    k_lm_step<TI, TO><<<grid, KCS_LM_TPB, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, (const TI *)theta_in, (TO *)theta_out, \
+                                                       (const TI *)lam_in, (TO *)lam_out, c->d_mask, c->d_vlist, c->n_inmask2, nvox, (double)gamma,  \
                                                        (double)delta, cost)
     if (!in_f64 && !out_f64) KCS_LM_GO(float, float);
     else if (!in_f64 && out_f64) KCS_LM_GO(float, double);
