@@ -112,6 +112,34 @@ def test_frame_ranges(pair):
     assert torch.equal(b_all, b_part)
 
 
+def test_no_cross_slice_or_border_leak(pair):
+    """Slices are independent direct planes and the padded borders must stay zero: with the neighbouring slices (and
+    frames) filled with 1e20 an out-of-slice tap or a clipped ray that reads past its slice shows up in the result."""
+    cfg, o, ctx = pair
+    T, nz = cfg["n_frames"], cfg["nz"]
+    if nz < 3:
+        pytest.skip("needs three slices")
+    x = np.float32(ki.uniform((T, nz, cfg["ny"], cfg["nx"]), seed=61, lo=0.0, hi=2.0)).astype(np.float64)
+    xb = x.copy()
+    xb[:, 0] *= 1e20
+    xb[:, 2] *= 1e20
+    y = torch.zeros((T, nz, cfg["n_angles"], cfg["n_bins"]), dtype=torch.float32, device="cuda")
+    ctx.forward_project(dev(xb), y)
+    yo = o.forward_project(x, -1)
+    assert rel_l2(host(y)[:, 1], yo[:, 1]) <= 1e-5
+    q = np.float32(ki.uniform(yo.shape, seed=62, lo=0.0, hi=2.0)).astype(np.float64)
+    qb = q.copy()
+    qb[:, 0] *= 1e20
+    qb[:, 2] *= 1e20
+    b = torch.zeros((T, nz, cfg["ny"], cfg["nx"]), dtype=torch.float32, device="cuda")
+    ctx.back_project(dev(qb), b)
+    bo = o.back_project(q, -1)
+    assert rel_l2(host(b)[:, 1], bo[:, 1]) <= 1e-5
+    # and a later ordinary call is unaffected by what the previous one left in the workspace
+    ctx.forward_project(dev(x), y)
+    assert rel_l2(host(y), yo) <= 1e-5
+
+
 def test_adjointness_gpu(pair):
     cfg, o, ctx = pair
     T = cfg["n_frames"]
