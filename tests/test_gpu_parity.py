@@ -140,6 +140,23 @@ def test_no_cross_slice_or_border_leak(pair):
     assert rel_l2(host(y), yo) <= 1e-5
 
 
+def test_bitwise_repeatable(pair):
+    """No atomics anywhere on the path (BJ north_star): two runs from the same state agree bit for bit."""
+    cfg, o, ctx = pair
+    mask = o.default_mask()
+    prob = ki.make_problem(cfg, mask, o.kinetic_eval, o.forward_project, noisy=True)
+    x0, th0, lam0 = ki.initial_state(cfg, mask, prob["y"], prob["r"], prob["scale"], o.forward_project)
+    y, r = dev(prob["y"]), dev(prob["r"])
+    outs = []
+    for _ in range(2):
+        x, th, lam = dev(x0), dev(th0), dev(lam0)
+        ctx.icm_iteration(y, r, float(prob["scale"]), x, th, lam, 0.0, cfg["gamma"], cfg["delta"], 2)
+        ctx.icm_iteration(y, r, float(prob["scale"]), x, th, lam, 0.1, cfg["gamma"], cfg["delta"], 2)
+        outs.append((x.clone(), th.clone(), lam.clone()))
+    for a, b in zip(*outs):
+        assert torch.equal(a, b)
+
+
 def test_adjointness_gpu(pair):
     cfg, o, ctx = pair
     T = cfg["n_frames"]
