@@ -12,7 +12,9 @@ projection, Poisson ratio, back-projection, OSL update) -> n_lm MAP-LM steps) on
   e2e        the same through kcs_icm_run_host with pinned HOST buffers: H2D of y, r, x, theta, lambda and D2H of
              x, theta, lambda inside the timed region.
   roofline   the dominant kernel class of the step (per-kernel CUDA events from kcs_profile_*, a second pass of K
-             steps): algorithmic flops / time against the FP32 FMA peak measured in this run.
+             steps): algorithmic flops / mean launch time against the FP32 FMA peak derived from
+             the SM count and clocks.max.sm (74.4 TFLOP/s); the FP32, FP64, L2 and L1 peaks measured in the same run by
+             kcs_probe_peak are printed beside it (`peaks_measured`).
   cpu_baseline  the fp64 oracle (oracle/, as it stands) on this box's host cores, one ICM iteration of the same workload.
   sweeps     C5(a)/(b) kernel sweeps on the C4 geometry (projector Gsamples/s by frames per launch, MAP-LM fits/s by
              gamma) and one C4 ICM iteration, unless --no-sweeps.

@@ -148,13 +148,6 @@ struct ProfScope {
 // straddle a 128 B line -- the L1 data pipe charges one wavefront per line touched by a request.
 static inline int round_up4(int n) { return n <= 4 ? 4 : n <= 8 ? 8 : n <= 16 ? 16 : 32; }
 
-// Frames-per-thread choice for a padded frame count Tp (multiple of 4): the largest of {16? no: 8, 12, 4}
-// that divides Tp, preferring 8 (register budget); FG = Tp / FPT lanes share one sample.
-static inline int choose_fpt(int Tp) {
-    (void)Tp;
-    return 4;  // one LDG.128 per lane and tap: the FG = Tp/4 lanes of a sample read its whole pixel in one request
-}
-
 // ---- launchers (kcs_projector.cu) ----------------------------------------------------------------
 // planar [nf][rows][W] (frame stride fs elements)  ->  inner [dst_index(row, col)][Tp]; frames >= nf are written 0.
 //   dst_index = (row / rps) * slab + (row % rps) * rstride + off + col

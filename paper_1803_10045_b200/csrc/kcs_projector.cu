@@ -267,7 +267,7 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
     FwdArgs p;
     p.xi = c->xi; p.qi = c->qi; p.yi = c->yi; p.ri = c->ri; p.r_pad = c->r_pad;
     p.Tp = Tp;
-    const int FPT = choose_fpt(Tp);
+    const int FPT = 4;  // one LDG.128 per lane and tap
     p.FG = Tp / FPT;
     p.As = subset < 0 ? g.A : g.A / g.S;
     p.subset = subset;
