@@ -129,9 +129,6 @@ struct FwdArgs {
 #ifndef KCS_FWD_TPB
 #define KCS_FWD_TPB 128
 #endif
-#ifndef KCS_BACK_ZBMAX
-#define KCS_BACK_ZBMAX 2
-#endif
 #ifndef KCS_BACK_MINBLK
 #define KCS_BACK_MINBLK 2
 #endif
@@ -510,37 +507,64 @@ __global__ void __launch_bounds__(256, KCS_BACK_MINBLK) k_back(KGeom g, BackArgs
     }
     if (!inimg) return;
 
-    const float smax = p.osl ? *p.smax : 0.f;
+    if (!p.osl) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+            if (!vin[v]) continue;
+            const int i = i0 + (v & 1), j = j0 + (v >> 1);
+#pragma unroll
+            for (int zb = 0; zb < ZB; ++zb) {
+                const int z = z0 + zb;
+                if (z >= g.nz) break;
+                const size_t o = (((size_t)z * g.nyp + (j + KCS_PAD)) * g.nxp + (i + KCS_PAD)) * Tp + fg * 4;
+                *reinterpret_cast<float4 *>(p.out + o) = make_float4(g.step_mm * acc[zb][v][0], g.step_mm * acc[zb][v][1],
+                                                                     g.step_mm * acc[zb][v][2], g.step_mm * acc[zb][v][3]);
+            }
+        }
+        return;
+    }
+    // O2 / eq. 2-3 with Q7-Q10:  x <- x * bp / max(S (1 + beta (x-F)/max(F,1e-20)), 0.1 S).  All x and F lines of the
+    // thread are requested first (they come from L2 / HBM), then updated and stored: one wait instead of 4 ZB.
+    const float smax = *p.smax;
     const float sc = p.scale * g.step_mm;
+    float4 xv[4][ZB], Fv[4][ZB];
+    float Sv[4];
+    bool live[4];
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+        const int i = min(i0 + (v & 1), g.nx - 1), j = min(j0 + (v >> 1), g.ny - 1);
+        const float S0 = p.sens[j * g.nx + i];
+        Sv[v] = p.scale * S0;
+        live[v] = vact[v] && (S0 > 1e-12f * smax);
+#pragma unroll
+        for (int zb = 0; zb < ZB; ++zb) {
+            const int z = min(z0 + zb, g.nz - 1);
+            const size_t o = (((size_t)z * g.nyp + (j + KCS_PAD)) * g.nxp + (i + KCS_PAD)) * Tp + fg * 4;
+            xv[v][zb] = make_float4(0.f, 0.f, 0.f, 0.f);
+            Fv[v][zb] = make_float4(1.f, 1.f, 1.f, 1.f);
+            if (live[v]) {
+                xv[v][zb] = *reinterpret_cast<const float4 *>(p.out + o);
+                Fv[v][zb] = __ldg(reinterpret_cast<const float4 *>(p.Fi + o));
+            }
+        }
+    }
 #pragma unroll
     for (int v = 0; v < 4; ++v) {
         if (!vin[v]) continue;
         const int i = i0 + (v & 1), j = j0 + (v >> 1);
-        const float S0 = p.osl ? p.sens[j * g.nx + i] : 0.f;
-        const float S = p.scale * S0;
-        const bool dead = (!vact[v]) || !(S0 > 1e-12f * smax);
 #pragma unroll
         for (int zb = 0; zb < ZB; ++zb) {
             const int z = z0 + zb;
             if (z >= g.nz) break;
             const size_t o = (((size_t)z * g.nyp + (j + KCS_PAD)) * g.nxp + (i + KCS_PAD)) * Tp + fg * 4;
-            if (!p.osl) {
-                *reinterpret_cast<float4 *>(p.out + o) = make_float4(g.step_mm * acc[zb][v][0], g.step_mm * acc[zb][v][1],
-                                                                     g.step_mm * acc[zb][v][2], g.step_mm * acc[zb][v][3]);
-            } else {
-                // O2 / eq. 2-3 with Q7-Q10:  x <- x * bp / max(S (1 + beta (x-F)/max(F,1e-20)), 0.1 S)
-                float4 xv = *reinterpret_cast<const float4 *>(p.out + o);
-                if (dead) {
-                    xv = make_float4(0.f, 0.f, 0.f, 0.f);
-                } else {
-                    const float4 Fv = __ldg(reinterpret_cast<const float4 *>(p.Fi + o));
-                    xv.x = osl_one(xv.x, sc * acc[zb][v][0], Fv.x, S, p.beta);
-                    xv.y = osl_one(xv.y, sc * acc[zb][v][1], Fv.y, S, p.beta);
-                    xv.z = osl_one(xv.z, sc * acc[zb][v][2], Fv.z, S, p.beta);
-                    xv.w = osl_one(xv.w, sc * acc[zb][v][3], Fv.w, S, p.beta);
-                }
-                *reinterpret_cast<float4 *>(p.out + o) = xv;
+            float4 out = make_float4(0.f, 0.f, 0.f, 0.f);  // outside the mask or without sensitivity: x = 0 (Q2, Q10)
+            if (live[v]) {
+                out.x = osl_one(xv[v][zb].x, sc * acc[zb][v][0], Fv[v][zb].x, Sv[v], p.beta);
+                out.y = osl_one(xv[v][zb].y, sc * acc[zb][v][1], Fv[v][zb].y, Sv[v], p.beta);
+                out.z = osl_one(xv[v][zb].z, sc * acc[zb][v][2], Fv[v][zb].z, Sv[v], p.beta);
+                out.w = osl_one(xv[v][zb].w, sc * acc[zb][v][3], Fv[v][zb].w, Sv[v], p.beta);
             }
+            *reinterpret_cast<float4 *>(p.out + o) = out;
         }
     }
 }
@@ -566,12 +590,11 @@ int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, f
     p.BY = nblk / p.BX;
     const int gx = (g.nx + 2 * p.BX - 1) / (2 * p.BX), gy = (g.ny + 2 * p.BY - 1) / (2 * p.BY);
     int ZB = 1;
-    if (KCS_BACK_ZBMAX >= 4 && g.nz >= 4 && (long long)gx * gy * ((g.nz + 3) / 4) >= 148LL) ZB = 4;
-    else if (g.nz >= 2 && (long long)gx * gy * ((g.nz + 1) / 2) >= 148LL) ZB = 2;
+    // ZB <= 2: the pipelined loop keeps the windows of all ZB slices (and the epilogue their x and F lines) in registers
+    if (g.nz >= 2 && (long long)gx * gy * ((g.nz + 1) / 2) >= 148LL) ZB = 2;
     dim3 grid(gx, gy, (g.nz + ZB - 1) / ZB);
     ProfScope ps(c, KCS_K_BACK);
     switch (ZB) {
-        case 4: k_back<4><<<grid, 256, 0, c->stream>>>(g, p); break;
         case 2: k_back<2><<<grid, 256, 0, c->stream>>>(g, p); break;
         default: k_back<1><<<grid, 256, 0, c->stream>>>(g, p); break;
     }
