@@ -198,7 +198,7 @@ int kcs_destroy(kcs_ctx *c) {
     if (!c) return KCS_ERR_NULL;
     cudaStreamSynchronize(c->stream);
     void *ptrs[] = {c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->d_wtab, c->d_vlist, c->xi, c->Fi,
-                    c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->thD[0], c->thD[1], c->lamD, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
+                    c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->thD[0], c->thD[1], c->lamD, c->lm_state, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     for (const KProfRec &r : c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -237,6 +237,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->d_vlist = nullptr; c->n_inmask2 = 0;
     c->xi = c->Fi = c->qi = c->yi = c->ri = c->r_pad = c->theta2 = nullptr;
     c->thD[0] = c->thD[1] = c->lamD = nullptr;
+    c->lm_state = nullptr;
     c->st_y = c->st_r = c->st_x = c->st_theta = c->st_lambda = nullptr;
     c->st_r_elems = 0;
 
@@ -347,6 +348,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     TRY(dalloc(c, &c->thD[0], 4 * c->n_vox));
     TRY(dalloc(c, &c->thD[1], 4 * c->n_vox));
     TRY(dalloc(c, &c->lamD, c->n_vox));
+    TRY(dalloc(c, &c->lm_state, (size_t)15 * (size_t)c->n_inmask2 * nz + 1));
     TRY(cudaMemcpyAsync(c->d_fwd, fw.data(), sizeof(double4) * A, cudaMemcpyHostToDevice, c->stream));
     TRY(cudaMemcpyAsync(c->d_bwd, bw.data(), sizeof(double4) * A, cudaMemcpyHostToDevice, c->stream));
     TRY(cudaMemcpyAsync(c->d_frames, frames.data(), sizeof(KFrame) * T, cudaMemcpyHostToDevice, c->stream));

@@ -100,6 +100,7 @@ struct kcs_ctx {
     float *theta2;  // [4][n_vox] fp32 scratch for a single Jacobi LM step (the caller's maps cannot be updated in place)
     double *thD[2]; // [4][n_vox] fp64 ping-pong buffers for the steps between the first and the last of a call
     double *lamD;   // [n_vox] lambda in fp64 between those steps
+    double *lm_state;  // [15][in-mask voxels] J^T J, J^T r, Phi_data of the current iterate, carried from step to step
     int xi_border_tp;  // Tp for which xi's zero border is valid (0 = unknown)
     float fov_rc2;     // (mask radius + 1.5 voxels)^2, mm^2: rays are clipped to this circle when x is known to be masked
 

@@ -245,6 +245,27 @@ __device__ __forceinline__ bool chol4(const double m[10], const double g[4], dou
     return true;
 }
 
+// Data part of the normal equations at theta: out[0..9] = J^T J (packed lower triangle), out[10..13] = J^T r,
+// out[14] = 1/2 sum r^2.  One (not inlined) copy of the model code serves both evaluations of a step.
+__device__ __forceinline__ void lm_eval(KKin kin, const KFrame *fr, const float *__restrict__ x, size_t xbase, size_t xstride,
+                                     double K1, double k2, double k3, double vB, double *out) {
+    double JtJ[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, gr[4] = {0, 0, 0, 0}, phi = 0.0;
+    tac_stream<true>(kin, fr, K1, k2, k3, vB, [&](int m, double Fm, double j0, double j1, double j2, double j3) {
+        const double r = (double)x[xbase + m * xstride] - Fm;
+        phi += 0.5 * r * r;
+        JtJ[0] += j0 * j0;
+        JtJ[1] += j1 * j0; JtJ[2] += j1 * j1;
+        JtJ[3] += j2 * j0; JtJ[4] += j2 * j1; JtJ[5] += j2 * j2;
+        JtJ[6] += j3 * j0; JtJ[7] += j3 * j1; JtJ[8] += j3 * j2; JtJ[9] += j3 * j3;
+        gr[0] += j0 * r; gr[1] += j1 * r; gr[2] += j2 * r; gr[3] += j3 * r;
+    });
+#pragma unroll
+    for (int q = 0; q < 10; ++q) out[q] = JtJ[q];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) out[10 + q] = gr[q];
+    out[14] = phi;
+}
+
 // 5 CTAs of 128 threads per SM (<= 102 registers): measured best of 1..8 on C2 and C4
 // TI / TO: storage type of the maps and of lambda on input / output.  Between the steps of one kcs_map_lm call the
 // iterate is kept in fp64 ping-pong buffers (TI = TO = double); only the caller's buffers are fp32.
@@ -261,7 +282,13 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
                                                  const TI *__restrict__ th_in, TO *__restrict__ th_out,
                                                  const TI *__restrict__ lam_in, TO *__restrict__ lam_out,
                                                  const unsigned char *__restrict__ mask, const int *__restrict__ vlist, int M2,
-                                                 long long nvox, double gamma, double delta, float *cost) {
+                                                 long long nvox, double gamma, double delta, float *cost,
+                                                 double *__restrict__ st, long long nfit) {
+    // FIRST step of a call (fp32 input): the data part of the normal equations is evaluated at theta.  Later steps read
+    // it from `st` [15][nfit], where the previous step left it for the iterate it produced: an accepted trial point was
+    // evaluated WITH its Jacobian, a rejected step leaves theta -- and therefore J^T J, J^T r, Phi_data -- unchanged.
+    // So a step costs one model + Jacobian evaluation instead of one with and one without.
+    constexpr bool FIRST = sizeof(TI) == 4, LAST = sizeof(TO) == 4;
     extern __shared__ double sh_raw[];
     KFrame *fr = reinterpret_cast<KFrame *>(sh_raw);
     load_frames(kin, fr);
@@ -294,30 +321,31 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
     }
     const XAddr xa = x_addr(g, (size_t)nvox, v, x_inner, Tp);
 
-    // pass 1: residual, J^T J, J^T r, Phi_old
-    double JtJ[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, gr[4] = {0, 0, 0, 0}, phi_old = 0.0;
-    tac_stream<true>(kin, fr, xi[0], xi[1], xi[2], xi[3], [&](int m, double Fm, double j0, double j1, double j2, double j3) {
-        const double r = (double)x[xa.base + m * xa.fstride] - Fm;
-        phi_old += 0.5 * r * r;
-        JtJ[0] += j0 * j0;
-        JtJ[1] += j1 * j0; JtJ[2] += j1 * j1;
-        JtJ[3] += j2 * j0; JtJ[4] += j2 * j1; JtJ[5] += j2 * j2;
-        JtJ[6] += j3 * j0; JtJ[7] += j3 * j1; JtJ[8] += j3 * j2; JtJ[9] += j3 * j3;
-        gr[0] += j0 * r; gr[1] += j1 * r; gr[2] += j2 * r; gr[3] += j3 * r;
-    });
+    double ev[15];
+    if (FIRST) {
+        lm_eval(kin, fr, x, xa.base, xa.fstride, xi[0], xi[1], xi[2], xi[3], ev);
+        if (!LAST) {
+#pragma unroll
+            for (int q = 0; q < 15; ++q) st[(size_t)q * nfit + t] = ev[q];  // kept if this step is rejected
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < 15; ++q) ev[q] = st[(size_t)q * nfit + t];
+    }
+    double gr[4] = {ev[10], ev[11], ev[12], ev[13]}, phi_old = ev[14];
     for (int q = 0; q < nn; ++q)
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
-            const double t = xi[p] - nb[q][p];
-            phi_old += gamma * huber(t, delta);
-            gr[p] -= gamma * huber_d(t, delta);
+            const double tt = xi[p] - nb[q][p];
+            phi_old += gamma * huber(tt, delta);
+            gr[p] -= gamma * huber_d(tt, delta);
         }
 
     double lam = lam_in[v];
-    if (!(lam > 0.0)) lam = 1e-3 * fmax(fmax(JtJ[0], JtJ[2]), fmax(JtJ[5], JtJ[9]));  // Q15 first use
+    if (!(lam > 0.0)) lam = 1e-3 * fmax(fmax(ev[0], ev[2]), fmax(ev[5], ev[9]));  // Q15 first use
     double M[10];
 #pragma unroll
-    for (int q = 0; q < 10; ++q) M[q] = JtJ[q];
+    for (int q = 0; q < 10; ++q) M[q] = ev[q];
     M[0] += lam; M[2] += lam; M[5] += lam; M[9] += lam;
     double d[4];
     double phi = phi_old;
@@ -328,11 +356,8 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
         double xt[4];
 #pragma unroll
         for (int p = 0; p < 4; ++p) xt[p] = fmin(fmax(xi[p] + d[p], lo[p]), hi[p]);
-        double phi_new = 0.0;
-        tac_stream<false>(kin, fr, xt[0], xt[1], xt[2], xt[3], [&](int m, double Fm, double, double, double, double) {
-            const double r = (double)x[xa.base + m * xa.fstride] - Fm;
-            phi_new += 0.5 * r * r;
-        });
+        lm_eval(kin, fr, x, xa.base, xa.fstride, xt[0], xt[1], xt[2], xt[3], ev);
+        double phi_new = ev[14];
         for (int q = 0; q < nn; ++q)
 #pragma unroll
             for (int p = 0; p < 4; ++p) phi_new += gamma * huber(xt[p] - nb[q][p], delta);
@@ -341,6 +366,10 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
             for (int p = 0; p < 4; ++p) xi[p] = xt[p];
             lam = fmax(lam / 10.0, 1e-30);
             phi = phi_new;
+            if (!LAST) {
+#pragma unroll
+                for (int q = 0; q < 15; ++q) st[(size_t)q * nfit + t] = ev[q];
+            }
         } else {
             lam = fmin(10.0 * lam, 1e30);
         }
@@ -374,7 +403,7 @@ int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const vo
 #define KCS_LM_GO(TI, TO)                                                                                              \
     k_lm_step<TI, TO><<<grid, KCS_LM_TPB, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, (const TI *)theta_in, (TO *)theta_out, \
                                                        (const TI *)lam_in, (TO *)lam_out, c->d_mask, c->d_vlist, c->n_inmask2, nvox, (double)gamma,  \
-                                                       (double)delta, cost)
+                                                       (double)delta, cost, c->lm_state, nfit)
     if (!in_f64 && !out_f64) KCS_LM_GO(float, float);
     else if (!in_f64 && out_f64) KCS_LM_GO(float, double);
     else if (in_f64 && out_f64) KCS_LM_GO(double, double);
