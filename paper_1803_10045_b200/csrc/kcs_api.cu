@@ -203,6 +203,8 @@ int kcs_destroy(kcs_ctx *c) {
         if (p) cudaFree(p);
     for (const KProfRec &r : c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
+    if (c->ev_x) cudaEventDestroy(c->ev_x);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
     return KCS_OK;
 }
@@ -238,6 +240,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->xi = c->Fi = c->qi = c->yi = c->ri = c->r_pad = c->theta2 = nullptr;
     c->thD[0] = c->thD[1] = c->lamD = nullptr;
     c->lm_state = nullptr;
+    c->ev_x = nullptr; c->copy_stream = nullptr;
     c->st_y = c->st_r = c->st_x = c->st_theta = c->st_lambda = nullptr;
     c->st_r_elems = 0;
 
@@ -463,8 +466,11 @@ int kcs_map_lm(kcs_ctx *c, const float *x, float *theta, float *lambda, float ga
     return lm_steps(c, x, 0, 0, theta, lambda, gamma, delta, n_steps, cost);
 }
 
-int kcs_icm_run(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta, float *lambda,
-                float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter) {
+// x_final (may be NULL): recorded on the context's stream as soon as the caller's x holds its final value, i.e. before
+// the last MAP-LM -- kcs_icm_run_host starts the device-to-host copy of x there, on a second stream, behind the fit.
+static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta,
+                        float *lambda, float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter,
+                        cudaEvent_t x_final) {
     if (!c) return KCS_ERR_NULL;
     if (!y || !r || !x || !theta || !lambda) return fail(c, KCS_ERR_NULL, "kcs_icm: NULL buffer");
     if (r_mode != KCS_R_PER_FRAME && r_mode != KCS_R_FULL) return fail(c, KCS_ERR_SHAPE, "kcs_icm: unknown r_mode");
@@ -496,9 +502,22 @@ int kcs_icm_run(kcs_ctx *c, const float *y, const float *r, int r_mode, float sc
             if ((rc = kcs_launch_forward(c, Tp, s, 1, scale, r_mode, (it > 0 || s > 0) ? 1 : 0))) return rc;
             if ((rc = kcs_launch_back(c, Tp, s, 1, nullptr, scale, b))) return rc;
         }
+        if (it == n_iter - 1) {  // the activity is final after the last OS pass; MAP-LM only reads it
+            if ((rc = unpack_image(c, c->xi, Tp, x, T))) return rc;
+            if (x_final) KCS_CUDA_OK(c, cudaEventRecord(x_final, c->stream));
+        }
         if ((rc = lm_steps(c, c->xi, 1, Tp, theta, lambda, gamma, delta, n_lm, nullptr))) return rc;
     }
-    return unpack_image(c, c->xi, Tp, x, T);
+    if (n_iter == 0) {
+        if ((rc = unpack_image(c, c->xi, Tp, x, T))) return rc;
+        if (x_final) KCS_CUDA_OK(c, cudaEventRecord(x_final, c->stream));
+    }
+    return KCS_OK;
+}
+
+int kcs_icm_run(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta, float *lambda,
+                float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter) {
+    return icm_run_impl(c, y, r, r_mode, scale, x, theta, lambda, beta_first, beta, gamma, delta, n_lm, n_iter, nullptr);
 }
 
 int kcs_icm_iteration(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta,
@@ -537,13 +556,20 @@ int kcs_icm_run_host(kcs_ctx *c, const float *y, const float *r, int r_mode, flo
     KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_x, x, nx_ * sizeof(float), cudaMemcpyHostToDevice, st));
     KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_theta, theta, 4 * c->n_vox * sizeof(float), cudaMemcpyHostToDevice, st));
     KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_lambda, lambda, c->n_vox * sizeof(float), cudaMemcpyHostToDevice, st));
-    int rc = kcs_icm_run(c, c->st_y, c->st_r, r_mode, scale, c->st_x, c->st_theta, c->st_lambda, beta_first, beta, gamma, delta,
-                         n_lm, n_iter);
+    if (!c->ev_x) {
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_x, cudaEventDisableTiming));
+        KCS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    }
+    int rc = icm_run_impl(c, c->st_y, c->st_r, r_mode, scale, c->st_x, c->st_theta, c->st_lambda, beta_first, beta, gamma, delta,
+                          n_lm, n_iter, c->ev_x);
     if (rc) return rc;
-    KCS_CUDA_OK(c, cudaMemcpyAsync(x, c->st_x, nx_ * sizeof(float), cudaMemcpyDeviceToHost, st));
+    // x goes back on a second stream while the last MAP-LM still runs on the first
+    KCS_CUDA_OK(c, cudaStreamWaitEvent(c->copy_stream, c->ev_x, 0));
+    KCS_CUDA_OK(c, cudaMemcpyAsync(x, c->st_x, nx_ * sizeof(float), cudaMemcpyDeviceToHost, c->copy_stream));
     KCS_CUDA_OK(c, cudaMemcpyAsync(theta, c->st_theta, 4 * c->n_vox * sizeof(float), cudaMemcpyDeviceToHost, st));
     KCS_CUDA_OK(c, cudaMemcpyAsync(lambda, c->st_lambda, c->n_vox * sizeof(float), cudaMemcpyDeviceToHost, st));
     KCS_CUDA_OK(c, cudaStreamSynchronize(st));
+    KCS_CUDA_OK(c, cudaStreamSynchronize(c->copy_stream));
     return KCS_OK;
 }
 

@@ -107,6 +107,8 @@ struct kcs_ctx {
     // device staging buffers of kcs_icm_run_host, allocated lazily
     float *st_y, *st_r, *st_x, *st_theta, *st_lambda;
     size_t st_r_elems;
+    cudaEvent_t ev_x;          // kcs_icm_run_host: x is final (recorded before the last MAP-LM)
+    cudaStream_t copy_stream;  // kcs_icm_run_host: device-to-host copy of x behind the last MAP-LM
 };
 
 #define KCS_CUDA_OK(ctx, call)                                                                  \
