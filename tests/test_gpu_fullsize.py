@@ -1,7 +1,7 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configurations bench.py times.
 
-C2 (the bench workload) is small enough for the oracle to run all 10 ICM iterations.  At the C4 geometry
-(344x344x127, 252x344, T = 29) the oracle computes a SLAB: direct planes are independent in the OS pass, and n LM
+C2 (the bench workload) is small enough for the oracle to run all 10 ICM iterations.  At the C3 and C4 geometries
+(128x128x64 / 168x128 and 344x344x127 / 252x344, T = 29) the oracle computes a SLAB: direct planes are independent in the OS pass, and n LM
 steps couple a slice to its n nearest neighbours only (Jacobi, 6-neighbourhood), so the centre slices of an
 8-slice slab that went through 3 LM steps are exactly what the full volume gives.  Every input comes from kcs_inputs
 and the oracle (never from the CUDA path); the GPU volume is the slab repeated along z.
@@ -79,10 +79,10 @@ def test_C2_icm_10_iterations_full_size():
     ctx.close()
 
 
-@pytest.fixture(scope="module")
-def c4_slab():
-    """8 central slices of the C4 phantom as an oracle problem, and the full C4 context."""
-    full = ki.config("C4")
+@pytest.fixture(scope="module", params=["C3", "C4"])
+def c4_slab(request):
+    """8 central slices of the C3 / C4 phantom as an oracle problem, and the full-size context."""
+    full = ki.config(request.param)
     ns = 8
     sub = dict(full, nz=ns, counts=full["counts"] * ns / full["nz"])
     o = Oracle(sub)
@@ -136,5 +136,5 @@ def test_C4_icm_iteration_on_slab(c4_slab):
     # the tiled volume is periodic in z except at its two ends: slab copy 1 (slices ns..2ns) sees periodic neighbours,
     # slab copy 0's centre slices 3, 4 see exactly the oracle's neighbours within 3 steps
     fr = frac_ok(host(th[:, 3:5]), tho[:, 3:5], mask)
-    print("C4 slab, iteration 1: parameter fractions (centre slices)", fr)
+    print(full["name"], "slab, iteration 1: parameter fractions (centre slices)", fr)
     assert min(fr) >= 0.999, fr

@@ -304,6 +304,26 @@ def test_map_lm(pair, gamma, delta, noise):
         assert np.array_equal(host(th)[:, :, ~m], start[:, :, ~m])  # out-of-mask voxels untouched
 
 
+@pytest.mark.parametrize("gamma", [0.0, 0.05, 0.5])
+def test_map_lm_c5b_recipe(gamma):
+    """BASELINE configs[4](b) on a small volume: 20 LM steps, start uniform within +/-50 % of the truth, gamma swept over
+    0, 0.05, 0.5 (noisy curves, three slices so that the z-neighbours take part)."""
+    cfg = ki.small_config(nx=40, ny=40, nz=3, n_angles=8, n_bins=40, n_subsets=2, sched="C3")
+    o = Oracle(cfg)
+    ctx = _kcs().Context(cfg)
+    mask, x, start, th_true = _lm_problem(cfg, o, 47, 0.15)
+    lam0 = np.zeros(x.shape[1:])
+    tho, lamo, costo = o.map_lm(x, start, lam0, gamma, 0.01, 20, want_cost=True)
+    th, lam = dev(start), dev(lam0)
+    cost = torch.zeros(x.shape[1:], dtype=torch.float32, device="cuda")
+    ctx.map_lm(dev(x), th, lam, gamma, 0.01, 20, cost)
+    fr = param_ok_fraction(host(th), tho, mask)
+    assert min(fr) >= 0.999, fr
+    m = mask > 0
+    assert np.mean(np.abs(host(cost)[:, m] - costo[:, m]) <= 1e-3 * np.abs(costo[:, m]) + 1e-6) >= 0.999
+    ctx.close()
+
+
 def test_map_lm_noiseless_recovers_truth():
     cfg = ki.config("C1")
     o = Oracle(cfg)
