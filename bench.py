@@ -108,8 +108,10 @@ def flops_model(cfg: dict) -> dict:
     sf_sub = T * nz * (A // S) * B * K        # sample-frames of one subset forward projection
     vaf_sub = T * nz * ny * nx * (A // S)     # voxel-angle-frames of one subset back-projection
     return {
-        "forward": {"units": sf_sub, "flop_per_unit": 8.0, "l2_bytes_per_unit": 4.0},  # 4 taps x 1 FMA
-        "back": {"units": vaf_sub, "flop_per_unit": 6.0, "l2_bytes_per_unit": 0.4},    # 3 merged bins x 1 FMA
+        # 4 taps x 1 FMA; every tap is a 4-byte read through L1 (16 B), every pixel-frame comes from L2 once per angle (4 B)
+        "forward": {"units": sf_sub, "flop_per_unit": 8.0, "l2_bytes_per_unit": 4.0, "l1_bytes_per_unit": 16.0},
+        # 3 merged bins x 1 FMA; the 2x2 block's 5-bin window is 5 lines per 4 voxels (5 B), ~0.4 B of it new from L2
+        "back": {"units": vaf_sub, "flop_per_unit": 6.0, "l2_bytes_per_unit": 0.4, "l1_bytes_per_unit": 5.0},
     }
 
 
@@ -279,6 +281,9 @@ def run_ours(args):
             result["peaks_measured"] = {k: ctx.probe_peak(k) for k in kcs.PEAK_PROBES}
             roofline["peak_measured_fp32_tflops"] = result["peaks_measured"]["fp32_tflops"]
             roofline["l2_achieved_gbs"] = fm[dom]["units"] * fm[dom]["l2_bytes_per_unit"] / (dom_ms * 1e-3) * 1e-9
+            # the unit that actually binds the projector pair: L1 data-pipe bytes against the L1 probe
+            roofline["l1_achieved_gbs"] = fm[dom]["units"] * fm[dom]["l1_bytes_per_unit"] / (dom_ms * 1e-3) * 1e-9
+            roofline["l1_frac_of_measured"] = roofline["l1_achieved_gbs"] / result["peaks_measured"]["l1_gbs"]
         except Exception as e:  # a probe failure must not lose the bench line
             result["peaks_measured"] = {"error": str(e)}
 

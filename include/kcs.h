@@ -100,6 +100,7 @@ int kcs_profile_read(kcs_ctx *ctx, double *ms, long long *count, int n_classes);
 #define KCS_PEAK_FP64_TFLOPS 1 /* the same with DFMA */
 #define KCS_PEAK_L2_GBS 2      /* L2-resident 32 MB buffer streamed by every CTA with ld.global.cg */
 #define KCS_PEAK_L1_GBS 3      /* 16 KB window per CTA re-read with coalesced LDG.128 (L1 hits) */
+#define KCS_PEAK_L2_GATHER_GBS 4 /* whole 128 B lines at random addresses of a 64 MB buffer (the projector's pattern) */
 int kcs_probe_peak(kcs_ctx *ctx, int what, double *out);
 
 /* P1-P3, P5 (BJ north_star "ray-driven parallel-beam line integrals with bilinear

@@ -26,7 +26,7 @@ PRIOR_ABSOLUTE = 1
 R_PER_FRAME = 0
 R_FULL = 1
 MAX_FRAMES = 32
-PEAK_PROBES = ("fp32_tflops", "fp64_tflops", "l2_gbs", "l1_gbs")
+PEAK_PROBES = ("fp32_tflops", "fp64_tflops", "l2_gbs", "l1_gbs", "l2_gather_gbs")
 PROFILE_CLASSES = ("pack", "unpack", "kinetic", "forward", "back", "lm", "other")
 
 # every symbol include/kcs.h declares (tests/test_abi.py checks the library exports each of them)
@@ -185,7 +185,7 @@ class Context:
         return {k: (float(ms[q]), int(n[q])) for q, k in enumerate(PROFILE_CLASSES)}
 
     def probe_peak(self, what: str) -> float:
-        """Measured machine peak: 'fp32_tflops', 'fp64_tflops', 'l2_gbs' or 'l1_gbs' (kcs_probe_peak)."""
+        """Measured machine peak: 'fp32_tflops', 'fp64_tflops', 'l2_gbs', 'l1_gbs' or 'l2_gather_gbs' (kcs_probe_peak)."""
         out = C.c_double(0.0)
         self._check(self._lib.kcs_probe_peak(self._h, PEAK_PROBES.index(what), C.byref(out)))
         return float(out.value)

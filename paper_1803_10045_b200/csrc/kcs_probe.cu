@@ -62,6 +62,27 @@ __global__ void __launch_bounds__(256) k_l1_read(const float4 *__restrict__ buf,
     if (s == -12345.f) out[0] = s;
 }
 
+// The projector's access pattern: every group of 8 lanes reads one whole 128 B line (LDG.128 each), 4 lines per warp
+// request, at pseudo-random line addresses of a 64 MB L2-resident buffer (no L1 reuse), 4 independent requests in flight.
+__global__ void __launch_bounds__(256) k_l2_gather(const float4 *__restrict__ buf, unsigned nlines, int iters, float *out) {
+    const unsigned gid = blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned grp = gid >> 3, lane8 = gid & 7;
+    unsigned h = grp * 2654435761u + 12345u;
+    float s = 0.f;
+    for (int i = 0; i < iters; ++i) {
+        float4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            h = h * 1664525u + 1013904223u;
+            const unsigned line = (h >> 8) % nlines;
+            v[u] = __ldg(buf + (size_t)line * 8 + lane8);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) s += v[u].x + v[u].y + v[u].z + v[u].w;
+    }
+    if (s == -12345.f) out[0] = s;
+}
+
 template <class Launch>
 int best_ms(kcs_ctx *c, Launch launch, float &best) {
     cudaEvent_t a, b;
@@ -126,6 +147,17 @@ extern "C" int kcs_probe_peak(kcs_ctx *c, int what, double *out) {
             const int iters = 1 << 12;
             rc = best_ms(c, [&] { k_l1_read<<<grid, 256, 0, c->stream>>>((const float4 *)scratch, iters, scratch); }, ms);
             *out = 16.0 * 4.0 * iters * 256.0 * grid / (ms * 1e-3) * 1e-9;
+            break;
+        }
+        case KCS_PEAK_L2_GATHER_GBS: {
+            float *big = nullptr;
+            const size_t bytes = 64u << 20;
+            KCS_CUDA_OK(c, cudaMalloc((void **)&big, bytes));
+            cudaMemsetAsync(big, 0, bytes, c->stream);
+            const int iters = 512;
+            rc = best_ms(c, [&] { k_l2_gather<<<grid, 256, 0, c->stream>>>((const float4 *)big, (unsigned)(bytes / 128), iters, scratch); }, ms);
+            *out = 16.0 * 4.0 * iters * 256.0 * grid / (ms * 1e-3) * 1e-9;
+            cudaFree(big);
             break;
         }
         default:
