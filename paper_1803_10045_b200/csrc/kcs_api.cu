@@ -205,6 +205,7 @@ int kcs_destroy(kcs_ctx *c) {
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
     if (c->ev_x) cudaEventDestroy(c->ev_x);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->aux_stream) { cudaStreamDestroy(c->aux_stream); cudaEventDestroy(c->ev_fork); cudaEventDestroy(c->ev_join); }
     delete c;
     return KCS_OK;
 }
@@ -241,6 +242,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->thD[0] = c->thD[1] = c->lamD = nullptr;
     c->lm_state = nullptr;
     c->ev_x = nullptr; c->copy_stream = nullptr;
+    c->aux_stream = nullptr; c->ev_fork = c->ev_join = nullptr;
     c->st_y = c->st_r = c->st_x = c->st_theta = c->st_lambda = nullptr;
     c->st_r_elems = 0;
 
@@ -466,6 +468,25 @@ int kcs_map_lm(kcs_ctx *c, const float *x, float *theta, float *lambda, float ga
     return lm_steps(c, x, 0, 0, theta, lambda, gamma, delta, n_steps, cost);
 }
 
+// F <- K(theta^{n-1}), held fixed during the pass ("one step late").  Only the OSL update needs F, so the evaluator
+// runs on a second stream, forked from everything enqueued so far and joined before the first back-projection.
+static int start_kinetic(kcs_ctx *c, const float *theta, int Tp) {
+    if (!c->aux_stream) {
+        KCS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+    }
+    cudaStream_t main_stream = c->stream;
+    KCS_CUDA_OK(c, cudaEventRecord(c->ev_fork, main_stream));
+    KCS_CUDA_OK(c, cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
+    c->stream = c->aux_stream;
+    const int rc = kcs_launch_kinetic(c, theta, c->Fi, nullptr, 1, Tp);
+    c->stream = main_stream;
+    if (rc) return rc;
+    KCS_CUDA_OK(c, cudaEventRecord(c->ev_join, c->aux_stream));
+    return KCS_OK;
+}
+
 // x_final (may be NULL): recorded on the context's stream as soon as the caller's x holds its final value, i.e. before
 // the last MAP-LM -- kcs_icm_run_host starts the device-to-host copy of x there, on a second stream, behind the fit.
 static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta,
@@ -478,6 +499,7 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
     const KGeom &g = c->g;
     const int T = c->cfg.n_frames, Tp = round_up4(T);
     int rc;
+    if (n_iter > 0 && (rc = start_kinetic(c, theta, Tp))) return rc;  // beside the packing and the first forward projection
     if ((rc = ensure_border(c, Tp))) return rc;
     if ((rc = pack_image(c, x, T, c->xi, Tp))) return rc;
     if ((rc = pack_sino(c, y, T, c->yi, Tp, g.A))) return rc;
@@ -495,11 +517,11 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
     }
     for (int it = 0; it < n_iter; ++it) {
         const float b = it == 0 ? beta_first : beta;
-        // F <- K(theta^{n-1}), held fixed during the pass ("one step late")
-        if ((rc = kcs_launch_kinetic(c, theta, c->Fi, nullptr, 1, Tp))) return rc;
+        if (it > 0 && (rc = start_kinetic(c, theta, Tp))) return rc;
         for (int s = 0; s < g.S; ++s) {  // Q5: subsets in order 0..S-1
             // after the first OSL update of this call x is zero outside the mask: rays are clipped to the FOV circle
             if ((rc = kcs_launch_forward(c, Tp, s, 1, scale, r_mode, (it > 0 || s > 0) ? 1 : 0))) return rc;
+            if (s == 0) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
             if ((rc = kcs_launch_back(c, Tp, s, 1, nullptr, scale, b))) return rc;
         }
         if (it == n_iter - 1) {  // the activity is final after the last OS pass; MAP-LM only reads it

@@ -108,6 +108,8 @@ struct kcs_ctx {
     float *st_y, *st_r, *st_x, *st_theta, *st_lambda;
     size_t st_r_elems;
     cudaEvent_t ev_x;          // kcs_icm_run_host: x is final (recorded before the last MAP-LM)
+    cudaStream_t aux_stream;   // kcs_icm_run: the kinetic evaluator runs here beside the first forward projection
+    cudaEvent_t ev_fork, ev_join;
     cudaStream_t copy_stream;  // kcs_icm_run_host: device-to-host copy of x behind the last MAP-LM
 };
 
