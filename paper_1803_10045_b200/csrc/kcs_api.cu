@@ -524,11 +524,20 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
             if (s == 0) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
             if ((rc = kcs_launch_back(c, Tp, s, 1, nullptr, scale, b))) return rc;
         }
-        if (it == n_iter - 1) {  // the activity is final after the last OS pass; MAP-LM only reads it
-            if ((rc = unpack_image(c, c->xi, Tp, x, T))) return rc;
-            if (x_final) KCS_CUDA_OK(c, cudaEventRecord(x_final, c->stream));
+        const bool last = it == n_iter - 1;
+        if (last) {  // the activity is final after the last OS pass; MAP-LM only reads it: unpack beside the fit
+            cudaStream_t main_stream = c->stream;
+            KCS_CUDA_OK(c, cudaEventRecord(c->ev_fork, main_stream));
+            KCS_CUDA_OK(c, cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
+            c->stream = c->aux_stream;
+            rc = unpack_image(c, c->xi, Tp, x, T);
+            c->stream = main_stream;
+            if (rc) return rc;
+            KCS_CUDA_OK(c, cudaEventRecord(c->ev_join, c->aux_stream));
+            if (x_final) KCS_CUDA_OK(c, cudaEventRecord(x_final, c->aux_stream));
         }
         if ((rc = lm_steps(c, c->xi, 1, Tp, theta, lambda, gamma, delta, n_lm, nullptr))) return rc;
+        if (last) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
     }
     if (n_iter == 0) {
         if ((rc = unpack_image(c, c->xi, Tp, x, T))) return rc;
