@@ -395,6 +395,43 @@ def test_projector_C2_full_size():
     ctx.close()
 
 
+def test_user_stream_ordering():
+    """Every call is enqueued on the stream given at create / kcs_set_stream and never synchronises: work issued on a
+    side stream (inputs prepared there, the second-stream overlap inside kcs_icm_iteration included) gives bit for bit
+    the default-stream result once that stream is synchronised."""
+    kcs = _kcs()
+    cfg = CONFIGS["ragged"]()
+    o = Oracle(cfg)
+    mask = o.default_mask()
+    prob = ki.make_problem(cfg, mask, o.kinetic_eval, o.forward_project, noisy=True)
+    x0, th0, lam0 = ki.initial_state(cfg, mask, prob["y"], prob["r"], prob["scale"], o.forward_project)
+    ref = kcs.Context(cfg)
+    y, r = dev(prob["y"]), dev(prob["r"])
+    xr, thr, lamr = dev(x0), dev(th0), dev(lam0)
+    for beta in (0.0, 0.1):
+        ref.icm_iteration(y, r, float(prob["scale"]), xr, thr, lamr, beta, cfg["gamma"], cfg["delta"], 3)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    ctx = kcs.Context(cfg, stream=side.cuda_stream)
+    with torch.cuda.stream(side):
+        xs, ths, lams = dev(x0), dev(th0), dev(lam0)       # produced on the side stream, consumed in order
+        for beta in (0.0, 0.1):
+            ctx.icm_iteration(y, r, float(prob["scale"]), xs, ths, lams, beta, cfg["gamma"], cfg["delta"], 3)
+    side.synchronize()
+    assert torch.equal(xs, xr) and torch.equal(ths, thr) and torch.equal(lams, lamr)
+    # moving the context to another stream later works the same way
+    other = torch.cuda.Stream()
+    ctx.set_stream(other.cuda_stream)
+    with torch.cuda.stream(other):
+        x2, th2, lam2 = dev(x0), dev(th0), dev(lam0)
+        for beta in (0.0, 0.1):
+            ctx.icm_iteration(y, r, float(prob["scale"]), x2, th2, lam2, beta, cfg["gamma"], cfg["delta"], 3)
+    other.synchronize()
+    assert torch.equal(x2, xr) and torch.equal(th2, thr)
+    ctx.close()
+    ref.close()
+
+
 def test_error_codes():
     kcs = _kcs()
     cfg = CONFIGS["tiny"]()
