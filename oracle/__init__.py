@@ -64,6 +64,8 @@ def _L():
         _lib.kcso_lm_objective.restype = d
         _lib.kcso_poisson_loglik.restype = d
         _lib.kcso_num_threads.restype = C.c_int
+        _lib.kcso_get_lm_accept_slack.restype = d
+        _lib.kcso_set_lm_accept_slack.argtypes = [d]
         _lib.kcso_ICp.argtypes = [vp, d]
         _lib.kcso_R.argtypes = [vp, d, d]
         _lib.kcso_G.argtypes = [vp, d, d]
@@ -79,6 +81,13 @@ def _p(a):
 def _f64(a):
     a = np.ascontiguousarray(a, dtype=np.float64)
     return a
+
+
+def set_lm_accept_slack(s: float) -> float:
+    """Q15a knob of the oracle (default 1e-6); returns the previous value."""
+    old = float(_L().kcso_get_lm_accept_slack())
+    _L().kcso_set_lm_accept_slack(float(s))
+    return old
 
 
 class Oracle:

@@ -82,6 +82,10 @@ double kcso_lm_objective(const kcso_config *c, const double *xv, const double xi
 void kcso_map_lm(const kcso_config *c, const double *x, double *theta, double *lambda,
                  double gamma, double delta, int n_steps, double *cost);
 
+/* Q15a knob (oracle only): relative slack of the LM acceptance test, default 1e-6. */
+void kcso_set_lm_accept_slack(double s);
+double kcso_get_lm_accept_slack(void);
+
 /* O1-O2 for all subsets in order 0..S-1 with F held fixed ("one OS-MAP-OSL pass"). r_mode 0: r[T] per-frame
  * constant, 1: r[T][nz][A][B] full sinogram. */
 void kcso_os_pass(const kcso_config *c, const double *y, const double *r, int r_mode, double scale,

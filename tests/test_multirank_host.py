@@ -21,7 +21,9 @@ mine = 1.0 + 0.5 * rank                       # rank 1 is the slow replica
 t = bench.max_over_ranks(mine, dist, torch.device("cpu"))
 v = bench.replica_throughput(world, 10, t)
 dist.barrier()
-print(json.dumps({{"rank": rank, "t": t, "value": v}}))
+# one file per rank: two ranks printing to one pipe can interleave inside a line
+with open(os.path.join({out!r}, "rank%d.json" % rank), "w") as f:
+    json.dump({{"rank": rank, "t": t, "value": v}}, f)
 dist.destroy_process_group()
 """
 
@@ -35,10 +37,10 @@ def _launch(code, extra_env=None, nproc=2, args=()):
 
 def test_time_is_max_over_ranks_and_value_counts_all_replicas(tmp_path):
     w = tmp_path / "worker.py"
-    w.write_text(WORKER.format(root=ROOT))
+    w.write_text(WORKER.format(root=ROOT, out=str(tmp_path)))
     r = _launch([str(w)])
     assert r.returncode == 0, r.stderr[-2000:]
-    rows = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    rows = [json.loads((tmp_path / f"rank{q}.json").read_text()) for q in range(2)]
     assert sorted(x["rank"] for x in rows) == [0, 1]
     for x in rows:
         assert x["t"] == pytest.approx(1.5)            # the slowest replica's time on every rank
