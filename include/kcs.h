@@ -17,8 +17,8 @@
  *        sinogram   y[T][nz][A][B]            subset sinogram  y_s[T][nz][A/S][B]  (local angle la <-> a = s + la*S)
  *        maps       theta[4][nz][ny][nx]      parameter order (K1, k2, k3, vB)
  *        lambda, cost [nz][ny][nx]
- *   - Internally the hot path keeps activity and sinograms frame-innermost ([voxel][Tp], Tp = T rounded
- *     up to a multiple of 4) so that one cache line fetched for a bilinear tap serves every time frame
+ *   - Internally the hot path keeps activity and sinograms frame-innermost ([voxel][Tp], Tp = the power
+ *     of two >= T, 4..32) so that one cache line fetched for a bilinear tap serves every time frame
  *     (BJ north_star); the pack/unpack transposes are part of the calls below.
  */
 #ifndef KCS_H
@@ -93,15 +93,6 @@ long long kcs_launch_count(const kcs_ctx *ctx);
 #define KCS_PROFILE_NCLASS 7
 int kcs_profile_enable(kcs_ctx *ctx, int on);
 int kcs_profile_read(kcs_ctx *ctx, double *ms, long long *count, int n_classes);
-
-/* Machine-peak microbenchmarks for the roofline denominators that MEASURED_PEAKS.json lacks:
- * runs a small kernel on the context's stream (best of 5, CUDA events), SYNCHRONISES, and writes *out [host]. */
-#define KCS_PEAK_FP32_TFLOPS 0 /* dependent-free FFMA chains, 2 flop per FMA */
-#define KCS_PEAK_FP64_TFLOPS 1 /* the same with DFMA */
-#define KCS_PEAK_L2_GBS 2      /* L2-resident 32 MB buffer streamed by every CTA with ld.global.cg */
-#define KCS_PEAK_L1_GBS 3      /* 16 KB window per CTA re-read with coalesced LDG.128 (L1 hits) */
-#define KCS_PEAK_L2_GATHER_GBS 4 /* whole 128 B lines at random addresses of a 64 MB buffer (the projector's pattern) */
-int kcs_probe_peak(kcs_ctx *ctx, int what, double *out);
 
 /* P1-P3, P5 (BJ north_star "ray-driven parallel-beam line integrals with bilinear
  * interpolation"):  y_s[f] = A_s x[f]  for frames f in [f0, f0+nf), all batched in one launch.

@@ -31,7 +31,7 @@ PROFILE_CLASSES = ("pack", "unpack", "kinetic", "forward", "back", "lm", "other"
 
 # every symbol include/kcs.h declares (tests/test_abi.py checks the library exports each of them)
 EXPORTS = ["kcs_create", "kcs_destroy", "kcs_set_stream", "kcs_last_error", "kcs_workspace_bytes", "kcs_get_mask",
-           "kcs_launch_count", "kcs_profile_enable", "kcs_profile_read", "kcs_probe_peak", "kcs_forward_project", "kcs_back_project", "kcs_sensitivity", "kcs_osl_update",
+           "kcs_launch_count", "kcs_profile_enable", "kcs_profile_read", "kcs_forward_project", "kcs_back_project", "kcs_sensitivity", "kcs_osl_update",
            "kcs_kinetic_eval", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host"]
 
 
@@ -86,7 +86,6 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.kcs_get_mask.argtypes = [vp, vp]
     lib.kcs_profile_enable.argtypes = [vp, i]
     lib.kcs_profile_read.argtypes = [vp, vp, vp, i]
-    lib.kcs_probe_peak.argtypes = [vp, i, C.POINTER(C.c_double)]
     lib.kcs_forward_project.argtypes = [vp, fp, fp, i, i, i]
     lib.kcs_back_project.argtypes = [vp, fp, fp, i, i, i]
     lib.kcs_sensitivity.argtypes = [vp, i, fp]
@@ -98,6 +97,21 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.kcs_icm_run_host.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, f, i, i]
     _lib = lib
     return lib
+
+
+def probe_peak(what: str, stream=None) -> float:
+    """BENCH-ONLY (libkcs_probe.so, include/kcs_probe.h): measured machine peak 'fp32_tflops', 'fp64_tflops', 'l2_gbs',
+    'l1_gbs' or 'l2_gather_gbs' on the current device."""
+    from . import build as _b
+    lib = C.CDLL(_b.build_probe())
+    lib.kcs_probe_peak.argtypes = [C.c_int, C.POINTER(C.c_double), C.c_void_p]
+    lib.kcs_probe_last_error.restype = C.c_char_p
+    out = C.c_double(0.0)
+    if stream is None:
+        stream = _torch().cuda.current_stream().cuda_stream
+    if lib.kcs_probe_peak(PEAK_PROBES.index(what), C.byref(out), C.c_void_p(stream)) != 0:
+        raise RuntimeError(lib.kcs_probe_last_error().decode())
+    return float(out.value)
 
 
 def _torch():
@@ -183,12 +197,6 @@ class Context:
         self._check(self._lib.kcs_profile_read(self._h, ms.ctypes.data_as(C.c_void_p), n.ctypes.data_as(C.c_void_p),
                                                len(PROFILE_CLASSES)))
         return {k: (float(ms[q]), int(n[q])) for q, k in enumerate(PROFILE_CLASSES)}
-
-    def probe_peak(self, what: str) -> float:
-        """Measured machine peak: 'fp32_tflops', 'fp64_tflops', 'l2_gbs', 'l1_gbs' or 'l2_gather_gbs' (kcs_probe_peak)."""
-        out = C.c_double(0.0)
-        self._check(self._lib.kcs_probe_peak(self._h, PEAK_PROBES.index(what), C.byref(out)))
-        return float(out.value)
 
     def mask(self) -> np.ndarray:
         m = np.zeros((self.ny, self.nx), dtype=np.uint8)

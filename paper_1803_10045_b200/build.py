@@ -1,4 +1,5 @@
-"""Build libkcs.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
+"""Build libkcs.so (the product) and libkcs_probe.so (bench-only peak probes) in-tree with nvcc for sm_100a
+(cross-compiles without a GPU)."""
 from __future__ import annotations
 
 import os
@@ -6,9 +7,13 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+INC = os.path.join(HERE, "..", "include")
 LIB = os.path.join(HERE, "libkcs.so")
-SOURCES = ["kcs_api.cu", "kcs_projector.cu", "kcs_kinetic.cu", "kcs_probe.cu"]
-HEADERS = [os.path.join(CSRC, "kcs_internal.cuh"), os.path.join(HERE, "..", "include", "kcs.h")]
+SOURCES = ["kcs_api.cu", "kcs_projector.cu", "kcs_kinetic.cu"]
+HEADERS = [os.path.join(CSRC, "kcs_internal.cuh"), os.path.join(INC, "kcs.h")]
+PROBE_LIB = os.path.join(HERE, "libkcs_probe.so")
+PROBE_SOURCES = [os.path.join("bench", "kcs_probe.cu")]
+PROBE_HEADERS = [os.path.join(INC, "kcs_probe.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
@@ -21,23 +26,36 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def is_stale() -> bool:
-    if not os.path.exists(LIB):
+def _stale(lib, sources, headers) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS
-    return any(os.path.getmtime(d) > t for d in deps)
+    t = os.path.getmtime(lib)
+    return any(os.path.getmtime(d) > t for d in [os.path.join(CSRC, s) for s in sources] + headers)
+
+
+def is_stale() -> bool:
+    return _stale(LIB, SOURCES, HEADERS)
+
+
+def _compile(lib, sources, verbose):
+    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", lib] + \
+          [os.path.join(CSRC, s) for s in sources]
+    subprocess.check_call(cmd)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or is_stale():
-        extra = os.environ.get("KCS_NVCC_EXTRA", "").split()  # developer knob: extra -D tuning macros
-        cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + \
-              [os.path.join(CSRC, s) for s in SOURCES]
-        subprocess.check_call(cmd)
+        _compile(LIB, SOURCES, verbose)
     return LIB
+
+
+def build_probe(force: bool = False, verbose: bool = False) -> str:
+    if force or _stale(PROBE_LIB, PROBE_SOURCES, PROBE_HEADERS):
+        _compile(PROBE_LIB, PROBE_SOURCES, verbose)
+    return PROBE_LIB
 
 
 if __name__ == "__main__":
     import sys
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build_probe(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,9 +1,15 @@
-// kcs_probe.cu -- machine-peak microbenchmarks behind kcs_probe_peak (include/kcs.h).
+// kcs_probe.cu -- machine-peak microbenchmarks behind kcs_probe_peak (include/kcs_probe.h).  BENCH-ONLY: built into
+// libkcs_probe.so, which bench.py loads for its roofline denominators; it is not part of libkcs.so and shares
+// nothing with it.
 //
 // MEASURED_PEAKS.json holds an HBM copy figure and a bf16 GEMM figure only; the rooflines that bound
 // this path (FP32 / FP64 FMA issue, L2->SM bandwidth, L1 bandwidth) must be measured on the box, in the same run
-// as the kernels they normalise.  Each probe is timed with CUDA events on the context's stream (best of 5).
-#include "kcs_internal.cuh"
+// as the kernels they normalise.  Each probe is timed with CUDA events on the given stream (best of 5).
+#include <cuda_runtime.h>
+
+#include <string>
+
+#include "../../../include/kcs_probe.h"
 
 namespace {
 
@@ -63,7 +69,8 @@ __global__ void __launch_bounds__(256) k_l1_read(const float4 *__restrict__ buf,
 }
 
 // The projector's access pattern: every group of 8 lanes reads one whole 128 B line (LDG.128 each), 4 lines per warp
-// request, at pseudo-random line addresses of a 64 MB L2-resident buffer (no L1 reuse), 4 independent requests in flight.
+// request, at pseudo-random line addresses of a 64 MB L2-resident buffer (ld.global.cg: L1 bypassed), 4 independent
+// requests in flight.
 __global__ void __launch_bounds__(256) k_l2_gather(const float4 *__restrict__ buf, unsigned nlines, int iters, float *out) {
     const unsigned gid = blockIdx.x * blockDim.x + threadIdx.x;
     const unsigned grp = gid >> 3, lane8 = gid & 7;
@@ -75,7 +82,7 @@ __global__ void __launch_bounds__(256) k_l2_gather(const float4 *__restrict__ bu
         for (int u = 0; u < 4; ++u) {
             h = h * 1664525u + 1013904223u;
             const unsigned line = (h >> 8) % nlines;
-            v[u] = __ldg(buf + (size_t)line * 8 + lane8);
+            v[u] = __ldcg(buf + (size_t)line * 8 + lane8);  // .cg: served by L2, never by the L1s in front of it
         }
 #pragma unroll
         for (int u = 0; u < 4; ++u) s += v[u].x + v[u].y + v[u].z + v[u].w;
@@ -83,21 +90,24 @@ __global__ void __launch_bounds__(256) k_l2_gather(const float4 *__restrict__ bu
     if (s == -12345.f) out[0] = s;
 }
 
+thread_local std::string g_err;
+
 template <class Launch>
-int best_ms(kcs_ctx *c, Launch launch, float &best) {
+int best_ms(cudaStream_t st, Launch launch, float &best) {
     cudaEvent_t a, b;
-    KCS_CUDA_OK(c, cudaEventCreate(&a));
-    KCS_CUDA_OK(c, cudaEventCreate(&b));
+    if (cudaEventCreate(&a) != cudaSuccess) { g_err = "cudaEventCreate failed"; return -1; }
+    if (cudaEventCreate(&b) != cudaSuccess) { cudaEventDestroy(a); g_err = "cudaEventCreate failed"; return -1; }
     best = 1e30f;
-    for (int rep = 0; rep < 6; ++rep) {  // first repetition warms up
-        cudaEventRecord(a, c->stream);
+    int rc = 0;
+    for (int rep = 0; rep < 6 && rc == 0; ++rep) {  // first repetition warms up
+        cudaEventRecord(a, st);
         launch();
-        cudaEventRecord(b, c->stream);
+        cudaEventRecord(b, st);
         cudaError_t e = cudaEventSynchronize(b);
         if (e != cudaSuccess) {
-            c->err = std::string("kcs_probe_peak: ") + cudaGetErrorString(e);
-            cudaEventDestroy(a); cudaEventDestroy(b);
-            return KCS_ERR_CUDA;
+            g_err = std::string("kcs_probe_peak: ") + cudaGetErrorString(e);
+            rc = -1;
+            break;
         }
         float t = 0.f;
         cudaEventElapsedTime(&t, a, b);
@@ -105,66 +115,75 @@ int best_ms(kcs_ctx *c, Launch launch, float &best) {
     }
     cudaEventDestroy(a);
     cudaEventDestroy(b);
-    return KCS_OK;
+    return rc;
 }
 
 }  // namespace
 
-extern "C" int kcs_probe_peak(kcs_ctx *c, int what, double *out) {
-    if (!c) return KCS_ERR_NULL;
-    if (!out) { c->err = "kcs_probe_peak: NULL out"; return KCS_ERR_NULL; }
+extern "C" const char *kcs_probe_last_error(void) { return g_err.c_str(); }
+
+extern "C" int kcs_probe_peak(int what, double *out, void *stream) {
+    if (!out) { g_err = "kcs_probe_peak: NULL out"; return -1; }
+    cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, sms = 0;
-    KCS_CUDA_OK(c, cudaGetDevice(&dev));
-    KCS_CUDA_OK(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        g_err = "kcs_probe_peak: no CUDA device";
+        return -1;
+    }
     const int grid = sms * 8;  // 8 CTAs of 256 threads per SM = 2048 resident threads
-    float *scratch = nullptr;
+    float *scratch = nullptr, *big = nullptr;
     const size_t l2_bytes = 32u << 20;  // well inside the 126 MB L2, far beyond the 256 KB L1s
-    KCS_CUDA_OK(c, cudaMalloc((void **)&scratch, l2_bytes));
-    cudaMemsetAsync(scratch, 0, l2_bytes, c->stream);
+    const size_t big_bytes = 64u << 20;
+    if (cudaMalloc((void **)&scratch, l2_bytes) != cudaSuccess ||
+        (what == KCS_PEAK_L2_GATHER_GBS && cudaMalloc((void **)&big, big_bytes) != cudaSuccess)) {
+        cudaGetLastError();
+        if (scratch) cudaFree(scratch);
+        g_err = "kcs_probe_peak: cudaMalloc failed";
+        return -1;
+    }
+    cudaMemsetAsync(scratch, 0, l2_bytes, st);
     float ms = 0.f;
-    int rc = KCS_OK;
+    int rc = 0;
     switch (what) {
         case KCS_PEAK_FP32_TFLOPS: {
             const int iters = 1 << 14;
-            rc = best_ms(c, [&] { k_fma_peak<float><<<grid, 256, 0, c->stream>>>(scratch, iters, 1.0f); }, ms);
+            rc = best_ms(st, [&] { k_fma_peak<float><<<grid, 256, 0, st>>>(scratch, iters, 1.0f); }, ms);
             *out = 2.0 * 8.0 * iters * 256.0 * grid / (ms * 1e-3) * 1e-12;
             break;
         }
         case KCS_PEAK_FP64_TFLOPS: {
             const int iters = 1 << 13;
-            rc = best_ms(c, [&] { k_fma_peak<double><<<grid, 256, 0, c->stream>>>((double *)scratch, iters, 1.0); }, ms);
+            rc = best_ms(st, [&] { k_fma_peak<double><<<grid, 256, 0, st>>>((double *)scratch, iters, 1.0); }, ms);
             *out = 2.0 * 8.0 * iters * 256.0 * grid / (ms * 1e-3) * 1e-12;
             break;
         }
         case KCS_PEAK_L2_GBS: {
             const int reps = 4;
             const size_t n4 = l2_bytes / 16;
-            rc = best_ms(c, [&] { k_l2_read<<<sms * 4, 256, 0, c->stream>>>((const float4 *)scratch, n4, reps, scratch); }, ms);
+            rc = best_ms(st, [&] { k_l2_read<<<sms * 4, 256, 0, st>>>((const float4 *)scratch, n4, reps, scratch); }, ms);
             *out = (double)l2_bytes * reps * (sms * 4) / (ms * 1e-3) * 1e-9;
             break;
         }
         case KCS_PEAK_L1_GBS: {
             const int iters = 1 << 12;
-            rc = best_ms(c, [&] { k_l1_read<<<grid, 256, 0, c->stream>>>((const float4 *)scratch, iters, scratch); }, ms);
+            rc = best_ms(st, [&] { k_l1_read<<<grid, 256, 0, st>>>((const float4 *)scratch, iters, scratch); }, ms);
             *out = 16.0 * 4.0 * iters * 256.0 * grid / (ms * 1e-3) * 1e-9;
             break;
         }
         case KCS_PEAK_L2_GATHER_GBS: {
-            float *big = nullptr;
-            const size_t bytes = 64u << 20;
-            KCS_CUDA_OK(c, cudaMalloc((void **)&big, bytes));
-            cudaMemsetAsync(big, 0, bytes, c->stream);
+            cudaMemsetAsync(big, 0, big_bytes, st);
             const int iters = 512;
-            rc = best_ms(c, [&] { k_l2_gather<<<grid, 256, 0, c->stream>>>((const float4 *)big, (unsigned)(bytes / 128), iters, scratch); }, ms);
+            rc = best_ms(st, [&] { k_l2_gather<<<grid, 256, 0, st>>>((const float4 *)big, (unsigned)(big_bytes / 128), iters, scratch); }, ms);
             *out = 16.0 * 4.0 * iters * 256.0 * grid / (ms * 1e-3) * 1e-9;
-            cudaFree(big);
             break;
         }
         default:
-            c->err = "kcs_probe_peak: unknown probe";
-            rc = KCS_ERR_SHAPE;
+            g_err = "kcs_probe_peak: unknown probe";
+            rc = -1;
     }
-    c->launches += (rc == KCS_OK) ? 6 : 0;
+    if (big) cudaFree(big);
     cudaFree(scratch);
     return rc;
 }

@@ -71,9 +71,9 @@ void fill_boundary(const Feng &fe, double t, KBoundary &b) {
 }
 
 int check_cfg(const kcs_config *c, std::string &why) {
-    if (c->nx <= 0 || c->ny <= 0 || c->nz <= 0 || c->n_angles <= 0 || c->n_bins < 3 || c->n_steps <= 0 ||
+    if (c->nx <= 0 || c->ny <= 0 || c->nz <= 0 || c->n_angles <= 0 || c->n_bins < 5 || c->n_steps <= 0 ||
         c->n_subsets <= 0 || !(c->vx > 0) || !(c->vy > 0) || !(c->bin_mm > 0) || !(c->step_mm > 0)) {
-        why = "non-positive size (n_bins must be >= 3)";
+        why = "non-positive size (n_bins must be >= 5: the back-projector reads 5-bin windows)";
         return KCS_ERR_SHAPE;
     }
     if (c->n_angles % c->n_subsets != 0) {
@@ -98,6 +98,11 @@ int check_cfg(const kcs_config *c, std::string &why) {
             why = "feng_lambda must be positive";
             return KCS_ERR_SHAPE;
         }
+    // the evaluator divides by a - lambda_1 without a series branch: lambda_1 must lie outside the rate box a = k2 + k3 <= 3 (Q16)
+    if (!(c->feng_lambda[0] > 3.05f)) {
+        why = "feng_lambda[0] must exceed 3.05 (it may not fall inside the rate box k2 + k3 <= 3)";
+        return KCS_ERR_SHAPE;
+    }
     for (int a = 0; a < c->n_angles; ++a) {
         const double th = M_PI * a / c->n_angles, cs = std::fabs(std::cos(th)), sn = std::fabs(std::sin(th));
         if ((cs * c->vx + sn * c->vy) / c->bin_mm > 1.5 || (sn * c->vx + cs * c->vy) / c->step_mm > 1.5) {

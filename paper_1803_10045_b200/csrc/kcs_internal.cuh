@@ -176,7 +176,7 @@ int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *se
 // ---- launchers (kcs_kinetic.cu) ------------------------------------------------------------------
 // F (and J) from theta.  inner == 0: F planar [T][V], J planar [4][T][V] or NULL;  inner == 1: F = padded inner layout, Tp.
 int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp);
-// one Jacobi LM step: reads theta_in, writes theta_out (all voxels; masked-out voxels are copied through).
+// one Jacobi LM step: reads theta_in, writes theta_out for the in-mask voxels (masked-out voxels are never touched).
 //   x_inner == 0: x planar [T][V];  x_inner == 1: x = c->xi padded inner layout with Tp.
 int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const void *theta_in, int in_f64, void *theta_out,
                        int out_f64, const void *lam_in, void *lam_out, float gamma, float delta, float *cost);

@@ -280,7 +280,7 @@ template <class TI, class TO>
 // of a slice.  Out-of-mask voxels get no thread (they are never read as neighbours and never written).
 __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, KKin kin, const float *__restrict__ x, int x_inner, int Tp,
                                                  const TI *__restrict__ th_in, TO *__restrict__ th_out,
-                                                 const TI *__restrict__ lam_in, TO *__restrict__ lam_out,
+                                                 const TI *lam_in, TO *lam_out,  // may alias: each thread touches its own element
                                                  const unsigned char *__restrict__ mask, const int *__restrict__ vlist, int M2,
                                                  long long nvox, double gamma, double delta, float *cost,
                                                  double *__restrict__ st, long long nfit) {

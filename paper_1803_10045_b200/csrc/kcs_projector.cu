@@ -154,6 +154,9 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, KCS_FWD_MINBLK) k_forward(KGeom g
     float acc[FPT];
 #pragma unroll
     for (int f = 0; f < FPT; ++f) acc[f] = 0.f;
+#ifdef KCS_EXP_ACC64
+    double accd[FPT] = {0.0, 0.0, 0.0, 0.0};
+#endif
 
     if (b < g.B) {
         const double4 fw = g.fwd[a];
@@ -193,6 +196,10 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, KCS_FWD_MINBLK) k_forward(KGeom g
             const double kk = (double)k0;
             int fxq = __double2int_rn(fma(kk, fw.y, pxa) * qs), fyq = __double2int_rn(fma(kk, fw.w, pya) * qs);
             const int mmax = min(KCS_ANCHOR, k_hi - k0);
+#ifdef KCS_EXP_ACC64
+            accd[0] += (double)acc[0]; accd[1] += (double)acc[1]; accd[2] += (double)acc[2]; accd[3] += (double)acc[3];
+            acc[0] = acc[1] = acc[2] = acc[3] = 0.f;
+#endif
 #pragma unroll(kUnroll)
             for (int m = 0; m < mmax; ++m) {
                 const int i0 = fxq >> FB, j0 = fyq >> FB;
@@ -213,6 +220,10 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, KCS_FWD_MINBLK) k_forward(KGeom g
         }
     }
 
+#ifdef KCS_EXP_ACC64
+#pragma unroll
+    for (int f = 0; f < FPT; ++f) acc[f] = (float)(accd[f] + (double)acc[f]);
+#endif
     // combine the KSPLIT partial sums of a ray (fixed order: deterministic)
     if (p.KSPLIT > 1) {
         const int nbf = p.BINS * FG;
@@ -346,7 +357,15 @@ __device__ __forceinline__ float4 voxel_angle_weights(const KGeom &g, int a, int
 __device__ __forceinline__ float osl_one(float x, float bp, float F, float S, float beta) {
     const float Fm = fmaxf(F, 1e-20f);
     const float den = S * fmaxf(fmaf(beta, x - F, Fm), 0.1f * Fm);
+#ifdef KCS_EXP_DIV
+    const float num = x * bp * Fm;
+    const float rc = __frcp_rn(den);
+    float q = num * rc;
+    q = fmaf(fmaf(-q, den, num), rc, q);
+    return q;
+#else
     return __fdividef(x * bp * Fm, den);
+#endif
 }
 
 struct BackArgs {

@@ -10,8 +10,8 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _header_functions():
-    src = open(os.path.join(ROOT, "include", "kcs.h")).read()
+def _header_functions(name="kcs.h"):
+    src = open(os.path.join(ROOT, "include", name)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(kcs_[a-z_0-9]+)\s*\(", src)))
 
@@ -25,6 +25,16 @@ def test_library_exports_every_declared_symbol():
     for n in names:
         assert hasattr(lib, n), n
     assert sorted(kcs.EXPORTS) == names
+    assert "kcs_probe_peak" not in names  # measuring tools are not part of the product ABI
+
+
+def test_every_header_has_its_library():
+    """include/ holds kcs.h (libkcs.so, the product) and kcs_probe.h (libkcs_probe.so, bench-only peak probes)."""
+    from paper_1803_10045_b200 import build as kb
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["kcs.h", "kcs_probe.h"]
+    lib = ctypes.CDLL(kb.build_probe())
+    for n in _header_functions("kcs_probe.h"):
+        assert hasattr(lib, n), n
 
 
 def test_built_for_sm_100a():
