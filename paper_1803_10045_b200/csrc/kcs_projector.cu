@@ -120,24 +120,12 @@ struct FwdArgs {
 };
 
 #define KCS_ANCHOR 16  // steps between fp64 re-anchoring of the sample coordinates
-#ifndef KCS_FWD_UNROLL
 #define KCS_FWD_UNROLL 4
-#endif
-#ifndef KCS_FWD_MINBLK
-#define KCS_FWD_MINBLK 1
-#endif
-#ifndef KCS_FWD_TPB
 #define KCS_FWD_TPB 128
-#endif
-#ifndef KCS_BACK_MINBLK
-#define KCS_BACK_MINBLK 2
-#endif
-#define KCS_STR2(x) #x
-#define KCS_STR(x) KCS_STR2(x)
 
 // One thread = one ray x 4 frames; the FG = Tp/4 lanes of a ray read a whole pixel (16 FG bytes) per tap in one request.
 template <int FG>
-__global__ void __launch_bounds__(KCS_FWD_TPB, KCS_FWD_MINBLK) k_forward(KGeom g, FwdArgs p) {
+__global__ void __launch_bounds__(KCS_FWD_TPB, 1) k_forward(KGeom g, FwdArgs p) {
     constexpr int FPT = 4, Tp = 4 * FG;
     // 16 loads in flight per thread pay when a warp covers few rays (FG >= 4); with 16-32 rays per warp the extra
     // registers cost more occupancy than the unrolling hides (C5(a) at 1 and 4 frames per launch)
@@ -154,9 +142,6 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, KCS_FWD_MINBLK) k_forward(KGeom g
     float acc[FPT];
 #pragma unroll
     for (int f = 0; f < FPT; ++f) acc[f] = 0.f;
-#ifdef KCS_EXP_ACC64
-    double accd[FPT] = {0.0, 0.0, 0.0, 0.0};
-#endif
 
     if (b < g.B) {
         const double4 fw = g.fwd[a];
@@ -191,15 +176,16 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, KCS_FWD_MINBLK) k_forward(KGeom g
         const int k_hi = (int)floor(thi) + 1;
         const int rowstride = g.nxp * Tp;
         const float *slice = p.xi + (size_t)z * g.nyp * rowstride + fg * FPT;
-        for (int k0 = k_lo; k0 < k_hi; k0 += KCS_ANCHOR) {
-            // fp64 anchor (P2): padded continuous index of sample (b, k0)
-            const double kk = (double)k0;
-            int fxq = __double2int_rn(fma(kk, fw.y, pxa) * qs), fyq = __double2int_rn(fma(kk, fw.w, pya) * qs);
-            const int mmax = min(KCS_ANCHOR, k_hi - k0);
-#ifdef KCS_EXP_ACC64
-            accd[0] += (double)acc[0]; accd[1] += (double)acc[1]; accd[2] += (double)acc[2]; accd[3] += (double)acc[3];
-            acc[0] = acc[1] = acc[2] = acc[3] = 0.f;
-#endif
+        // Anchor blocks sit on the absolute grid k = 0, 16, 32, ...: the fixed-point coordinates of sample k do not depend
+        // on where clipping (or the K-split) starts the walk, so a clipped and an unclipped projection of an image that is
+        // zero outside the field of view agree bit for bit.
+        for (int kb = (k_lo / KCS_ANCHOR) * KCS_ANCHOR; kb < k_hi; kb += KCS_ANCHOR) {
+            // fp64 anchor (P2): padded continuous index of sample (b, kb), advanced exactly to the first sample of the walk
+            const double kk = (double)kb;
+            const int k0 = max(kb, k_lo);
+            int fxq = __double2int_rn(fma(kk, fw.y, pxa) * qs) + (k0 - kb) * dxq;
+            int fyq = __double2int_rn(fma(kk, fw.w, pya) * qs) + (k0 - kb) * dyq;
+            const int mmax = min(kb + KCS_ANCHOR, k_hi) - k0;
 #pragma unroll(kUnroll)
             for (int m = 0; m < mmax; ++m) {
                 const int i0 = fxq >> FB, j0 = fyq >> FB;
@@ -220,10 +206,6 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, KCS_FWD_MINBLK) k_forward(KGeom g
         }
     }
 
-#ifdef KCS_EXP_ACC64
-#pragma unroll
-    for (int f = 0; f < FPT; ++f) acc[f] = (float)(accd[f] + (double)acc[f]);
-#endif
     // combine the KSPLIT partial sums of a ray (fixed order: deterministic)
     if (p.KSPLIT > 1) {
         const int nbf = p.BINS * FG;
@@ -316,6 +298,9 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
 //   the sample map; only samples b in rint(fb)+{-1,0,1}, k in rint(fk)+{-1,0,1} can lie inside the voxel's tent
 //   support (kcs_create checks the geometry ratio that guarantees this).  w_b = sum_k tent(dx) tent(dy).
 // ---------------------------------------------------------------------------------------------------------
+// Evaluated in fp64 (a geometry-only table, built once per context): a weight at the edge of a tent is a difference
+// 1 - |d| of nearly equal numbers, and at low counts a voxel's update can hinge on that one weight (every other bin it
+// sees holds y = 0), so the weights must be accurate RELATIVE to themselves, not to 1.
 __device__ __forceinline__ float4 voxel_angle_weights(const KGeom &g, int a, int i, int j) {
     const double4 q = g.bwd[a];
     const double4 fw = g.fwd[a];
@@ -323,21 +308,20 @@ __device__ __forceinline__ float4 voxel_angle_weights(const KGeom &g, int a, int
     const double fb = fma(xc, q.x, fma(yc, q.y, g.cb));
     const double fk = fma(xc, q.z, fma(yc, q.w, g.ck));
     const double rb = rint(fb), rk = rint(fk);
-    const float db0 = (float)(rb - fb), dk0 = (float)(rk - fk);
+    const double db0 = rb - fb, dk0 = rk - fk;
     const int b1 = (int)rb, k1 = (int)rk;
-    const float axb = (float)fw.x, axk = (float)fw.y, ayb = (float)fw.z, ayk = (float)fw.w;
-    float w[3] = {0.f, 0.f, 0.f};
+    double w[3] = {0.0, 0.0, 0.0};
 #pragma unroll
     for (int sk = -1; sk <= 1; ++sk) {
         const int k = k1 + sk;
         const bool kvalid = (k >= 0) && (k < g.K);
-        const float dk = dk0 + (float)sk;
+        const double dk = dk0 + (double)sk;
 #pragma unroll
         for (int sb = -1; sb <= 1; ++sb) {
-            const float db = db0 + (float)sb;
-            const float dx = fmaf(db, axb, dk * axk), dy = fmaf(db, ayb, dk * ayk);
-            const float t = fmaxf(0.f, 1.f - fabsf(dx)) * fmaxf(0.f, 1.f - fabsf(dy));
-            w[sb + 1] += kvalid ? t : 0.f;
+            const double db = db0 + (double)sb;
+            const double dx = fma(db, fw.x, dk * fw.y), dy = fma(db, fw.z, dk * fw.w);
+            const double t = fmax(0.0, 1.0 - fabs(dx)) * fmax(0.0, 1.0 - fabs(dy));
+            w[sb + 1] += kvalid ? t : 0.0;
         }
     }
     // re-align to a base bin b0c in [0, B-3] so the three loads never leave the row
@@ -347,7 +331,7 @@ __device__ __forceinline__ float4 voxel_angle_weights(const KGeom &g, int a, int
 #pragma unroll
     for (int r = 0; r < 3; ++r) {
         const int rr = b0c + r - b0;
-        wo[r] = (rr == 0) ? w[0] : (rr == 1) ? w[1] : (rr == 2) ? w[2] : 0.f;
+        wo[r] = (float)((rr == 0) ? w[0] : (rr == 1) ? w[1] : (rr == 2) ? w[2] : 0.0);
     }
     return make_float4(__int_as_float(b0c), wo[0], wo[1], wo[2]);
 }
@@ -357,15 +341,7 @@ __device__ __forceinline__ float4 voxel_angle_weights(const KGeom &g, int a, int
 __device__ __forceinline__ float osl_one(float x, float bp, float F, float S, float beta) {
     const float Fm = fmaxf(F, 1e-20f);
     const float den = S * fmaxf(fmaf(beta, x - F, Fm), 0.1f * Fm);
-#ifdef KCS_EXP_DIV
-    const float num = x * bp * Fm;
-    const float rc = __frcp_rn(den);
-    float q = num * rc;
-    q = fmaf(fmaf(-q, den, num), rc, q);
-    return q;
-#else
     return __fdividef(x * bp * Fm, den);
-#endif
 }
 
 struct BackArgs {
@@ -437,7 +413,7 @@ int kcs_launch_build_wtab(kcs_ctx *c) {
 // voxels: 1.25 L1 wavefronts per voxel-angle instead of 3.  Weights come from the k_build_wtab table (L2 resident:
 // it is the same for every slice and frame).  No atomics: run-to-run deterministic.
 template <int ZB>
-__global__ void __launch_bounds__(256, KCS_BACK_MINBLK) k_back(KGeom g, BackArgs p) {
+__global__ void __launch_bounds__(256, 2) k_back(KGeom g, BackArgs p) {
     const int tid = threadIdx.x;
     const int fg = tid % p.FG;
     const int blk = tid / p.FG;
@@ -630,13 +606,13 @@ __global__ void k_sens(KGeom g, float *sens, float *smax) {
     const int s = blockIdx.z;  // s == S: all angles
     if (i >= g.nx) return;
     const int As = s == g.S ? g.A : g.A / g.S;
-    float sum = 0.f;
+    double acc = 0.0;
     for (int la = 0; la < As; ++la) {
         const int a = s == g.S ? la : s + la * g.S;
         const float4 w = voxel_angle_weights(g, a, i, j);
-        sum += w.y + w.z + w.w;
+        acc += (double)w.y + (double)w.z + (double)w.w;
     }
-    sum *= g.step_mm;
+    const float sum = (float)(acc * (double)g.step_mm);
     sens[((size_t)s * g.ny + j) * g.nx + i] = sum;
     atomicMax(reinterpret_cast<int *>(smax + s), __float_as_int(sum));  // sum >= 0: int order == float order
 }

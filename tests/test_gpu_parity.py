@@ -34,6 +34,13 @@ def rel_l2(g, o):
     return float(np.linalg.norm((g - o).ravel()) / max(np.linalg.norm(o.ravel()), 1e-300))
 
 
+def close(g, o, tol):
+    """BJ's tolerance is a relative L2; a whole-array norm hides a wrong edge bin or border voxel, so every parity check
+    also bounds the largest element-wise error: max|g - o| <= tol max|o|."""
+    g, o = np.asarray(g), np.asarray(o)
+    return rel_l2(g, o) <= tol and float(np.abs(g - o).max()) <= tol * float(np.abs(o).max())
+
+
 def param_ok_fraction(thg, tho, mask):
     ok = np.abs(thg - tho) <= 1e-3 * np.maximum(np.abs(tho), FLOORS[:, None, None, None])
     return [float(ok[p][:, mask > 0].mean()) for p in range(4)]
@@ -74,10 +81,10 @@ def test_forward_project(pair, subset):
     yo = o.forward_project(x32, subset)
     y = torch.zeros(yo.shape, dtype=torch.float32, device="cuda")
     ctx.forward_project(dev(x32), y, subset)
-    assert rel_l2(host(y), yo) <= 1e-5
+    assert close(host(y), yo, 1e-5)
     # per-frame too (a frame must not leak into its neighbour)
     for f in (0, T - 1):
-        assert rel_l2(host(y)[f], yo[f]) <= 1e-5
+        assert close(host(y)[f], yo[f], 1e-5)
 
 
 @pytest.mark.parametrize("subset", [-1, 1])
@@ -89,8 +96,8 @@ def test_back_project(pair, subset):
     bo = o.back_project(q, subset)
     b = torch.zeros(bo.shape, dtype=torch.float32, device="cuda")
     ctx.back_project(dev(q), b, subset)
-    assert rel_l2(host(b), bo) <= 1e-5
-    assert rel_l2(host(b)[T - 1], bo[T - 1]) <= 1e-5
+    assert close(host(b), bo, 1e-5)
+    assert close(host(b)[T - 1], bo[T - 1], 1e-5)
 
 
 def test_frame_ranges(pair):
@@ -126,7 +133,7 @@ def test_no_cross_slice_or_border_leak(pair):
     y = torch.zeros((T, nz, cfg["n_angles"], cfg["n_bins"]), dtype=torch.float32, device="cuda")
     ctx.forward_project(dev(xb), y)
     yo = o.forward_project(x, -1)
-    assert rel_l2(host(y)[:, 1], yo[:, 1]) <= 1e-5
+    assert close(host(y)[:, 1], yo[:, 1], 1e-5)
     q = np.float32(ki.uniform(yo.shape, seed=62, lo=0.0, hi=2.0)).astype(np.float64)
     qb = q.copy()
     qb[:, 0] *= 1e20
@@ -134,10 +141,10 @@ def test_no_cross_slice_or_border_leak(pair):
     b = torch.zeros((T, nz, cfg["ny"], cfg["nx"]), dtype=torch.float32, device="cuda")
     ctx.back_project(dev(qb), b)
     bo = o.back_project(q, -1)
-    assert rel_l2(host(b)[:, 1], bo[:, 1]) <= 1e-5
+    assert close(host(b)[:, 1], bo[:, 1], 1e-5)
     # and a later ordinary call is unaffected by what the previous one left in the workspace
     ctx.forward_project(dev(x), y)
-    assert rel_l2(host(y), yo) <= 1e-5
+    assert close(host(y), yo, 1e-5)
 
 
 def test_bitwise_repeatable(pair):
@@ -176,7 +183,7 @@ def test_sensitivity(pair):
     for s in (-1, 0, cfg["n_subsets"] - 1):
         sg = torch.zeros((cfg["ny"], cfg["nx"]), dtype=torch.float32, device="cuda")
         ctx.sensitivity(s, sg)
-        assert rel_l2(host(sg), o.sensitivity(s)) <= 1e-5
+        assert close(host(sg), o.sensitivity(s), 1e-5)
 
 
 @pytest.mark.parametrize("mode", [0, 1])
@@ -192,7 +199,7 @@ def test_osl_update(pair, mode):
     xo = o.osl_update(x, bp, sens, F, 0.1, mode, 2.5)
     xg = dev(x)
     ctx.osl_update(xg, dev(bp), dev(sens), dev(F), 0.1, mode, 2.5)
-    assert rel_l2(host(xg), xo) <= 1e-5
+    assert close(host(xg), xo, 1e-5)
     m = ctx.mask()
     assert np.all(host(xg)[:, :, m == 0] == 0)
 
@@ -210,7 +217,7 @@ def test_one_os_pass_through_icm(pair):
                                      x0, th0, lam0, beta, 0.0, 0.01, 0)
         x, th, lam = dev(x0), dev(th0), dev(lam0)
         ctx.icm_iteration(dev(prob["y"]), dev(prob["r"]), float(prob["scale"]), x, th, lam, beta, 0.0, 0.01, 0)
-        assert rel_l2(host(x), xo) <= 1e-4
+        assert close(host(x), xo, 1e-4)
         assert np.array_equal(host(th), tho)
         # full randoms sinogram gives the same result as the per-frame constant
         rfull = np.broadcast_to(np.float32(prob["r"])[:, None, None, None], prob["y"].shape)
@@ -366,8 +373,7 @@ def test_icm_10_iterations(name):
     # kcs_icm_run (y packed once) and the host-buffer entry give the same iterates as 10 single calls
     x2, th2, lam2 = dev(x0), dev(th0), dev(lam0)
     ctx.icm_run(y, rd, scale, x2, th2, lam2, 0.0, cfg["beta"], cfg["gamma"], cfg["delta"], cfg["n_lm"], cfg["n_icm"])
-    assert rel_l2(host(x2), host(x)) <= 1e-5
-    assert min(param_ok_fraction(host(th2), host(th), mask)) >= 0.999
+    assert torch.equal(x2, x) and torch.equal(th2, th) and torch.equal(lam2, lam)  # bit for bit: same kernels, same order
     hx, hth, hlam = np.float32(x0), np.float32(th0), np.float32(lam0)
     ctx.icm_run_host(np.float32(prob["y"]), np.float32(r), scale, hx, hth, hlam, 0.0, cfg["beta"], cfg["gamma"],
                      cfg["delta"], cfg["n_lm"], cfg["n_icm"])
@@ -386,12 +392,12 @@ def test_projector_C2_full_size():
     yo = o.forward_project(x, -1)
     y = torch.zeros(yo.shape, dtype=torch.float32, device="cuda")
     ctx.forward_project(dev(x), y)
-    assert rel_l2(host(y), yo) <= 1e-5
+    assert close(host(y), yo, 1e-5)
     q = np.float32(ki.uniform(yo.shape, seed=52)).astype(np.float64)
     bo = o.back_project(q, -1)
     b = torch.zeros(x.shape, dtype=torch.float32, device="cuda")
     ctx.back_project(dev(q), b)
-    assert rel_l2(host(b), bo) <= 1e-5
+    assert close(host(b), bo, 1e-5)
     ctx.close()
 
 
