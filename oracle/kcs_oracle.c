@@ -43,6 +43,25 @@ static void sample_index(const kcso_config *c, double cs, double sn, int b, int 
     *fy = Y / c->vy + 0.5 * (double)(c->ny - 1);
 }
 
+/* Q23: a sample within KCSO_SNAP of a pixel centre (in pixel units) is taken to lie ON it.  At
+ * 0 and 90 degrees with bin = step = voxel every sample of P2 falls exactly on a pixel centre, but fx is computed with
+ * ~1e-14 of rounding, which leaves a weight of ~1e-14 on the neighbouring pixel; P2's interpolant has no such term. At
+ * low counts a voxel's OSL update can hinge on that one spurious weight (every bin it really sees holds y = 0), and the
+ * iteration amplifies it by 20 orders of magnitude within one pass: the iterate would depend on the oracle's own rounding.
+ * The split into (floor, fraction) is the only place the snap enters; forward and transposed projector share it, so
+ * A^T stays the exact transpose of A. */
+#ifndef KCSO_SNAP
+#define KCSO_SNAP 1e-9
+#endif
+static void split_index(double f, int *i0, double *w) {
+    const double fl = floor(f);
+    double fr = f - fl;
+    if (fr < KCSO_SNAP) fr = 0.0;
+    else if (fr > 1.0 - KCSO_SNAP) fr = 1.0;
+    *i0 = (int)fl;
+    *w = fr;
+}
+
 static int subset_count(const kcso_config *c, int subset) {
     return subset < 0 ? c->n_angles : c->n_angles / c->n_subsets;
 }
@@ -101,8 +120,10 @@ void kcso_forward_project(const kcso_config *c, const double *x, double *y, int 
                 for (int k = 0; k < c->n_steps; ++k) {
                     double fx, fy;
                     sample_index(c, cs, sn, b, k, &fx, &fy);
-                    const int i0 = (int)floor(fx), j0 = (int)floor(fy);
-                    const double wx = fx - (double)i0, wy = fy - (double)j0;
+                    int i0, j0;
+                    double wx, wy;
+                    split_index(fx, &i0, &wx);
+                    split_index(fy, &j0, &wy);
                     acc += (1.0 - wx) * (1.0 - wy) * pix(img, c->nx, c->ny, i0, j0) +
                            wx * (1.0 - wy) * pix(img, c->nx, c->ny, i0 + 1, j0) +
                            (1.0 - wx) * wy * pix(img, c->nx, c->ny, i0, j0 + 1) +
@@ -128,8 +149,10 @@ static void back_project_slice(const kcso_config *c, const double *sino, double 
             for (int k = 0; k < c->n_steps; ++k) {
                 double fx, fy;
                 sample_index(c, cs, sn, b, k, &fx, &fy);
-                const int i0 = (int)floor(fx), j0 = (int)floor(fy);
-                const double wx = fx - (double)i0, wy = fy - (double)j0;
+                int i0, j0;
+                double wx, wy;
+                split_index(fx, &i0, &wx);
+                split_index(fy, &j0, &wy);
                 const double w[4] = {(1.0 - wx) * (1.0 - wy), wx * (1.0 - wy), (1.0 - wx) * wy, wx * wy};
                 const int ii[4] = {i0, i0 + 1, i0, i0 + 1};
                 const int jj[4] = {j0, j0, j0 + 1, j0 + 1};

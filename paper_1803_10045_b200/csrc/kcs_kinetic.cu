@@ -270,12 +270,8 @@ __device__ __forceinline__ void lm_eval(KKin kin, const KFrame *fr, const float 
 // TI / TO: storage type of the maps and of lambda on input / output.  Between the steps of one kcs_map_lm call the
 // iterate is kept in fp64 ping-pong buffers (TI = TO = double); only the caller's buffers are fp32.
 template <class TI, class TO>
-#ifndef KCS_LM_TPB
 #define KCS_LM_TPB 128
-#endif
-#ifndef KCS_LM_MINBLK
 #define KCS_LM_MINBLK 5
-#endif
 // One thread per IN-MASK voxel: thread t of the launch fits voxel (z = t / M2, pixel vlist[t % M2]), M2 = in-mask pixels
 // of a slice.  Out-of-mask voxels get no thread (they are never read as neighbours and never written).
 __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, KKin kin, const float *__restrict__ x, int x_inner, int Tp,

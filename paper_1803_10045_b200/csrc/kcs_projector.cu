@@ -298,6 +298,14 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
 //   the sample map; only samples b in rint(fb)+{-1,0,1}, k in rint(fk)+{-1,0,1} can lie inside the voxel's tent
 //   support (kcs_create checks the geometry ratio that guarantees this).  w_b = sum_k tent(dx) tent(dy).
 // ---------------------------------------------------------------------------------------------------------
+// Tent weight with reading Q23: a sample within 1e-9 pixel of a pixel centre lies ON it, so the weight
+// is exactly 1 there and exactly 0 on the neighbours one pixel away (at 0 and 90 degrees every sample is such a sample;
+// without the snap the weight left on the neighbour is rounding residue of ~1e-14).
+__device__ __forceinline__ double tent_q23(double d) {
+    const double ad = fabs(d);
+    return ad < 1e-9 ? 1.0 : (ad > 1.0 - 1e-9 ? 0.0 : 1.0 - ad);
+}
+
 // Evaluated in fp64 (a geometry-only table, built once per context): a weight at the edge of a tent is a difference
 // 1 - |d| of nearly equal numbers, and at low counts a voxel's update can hinge on that one weight (every other bin it
 // sees holds y = 0), so the weights must be accurate RELATIVE to themselves, not to 1.
@@ -320,7 +328,7 @@ __device__ __forceinline__ float4 voxel_angle_weights(const KGeom &g, int a, int
         for (int sb = -1; sb <= 1; ++sb) {
             const double db = db0 + (double)sb;
             const double dx = fma(db, fw.x, dk * fw.y), dy = fma(db, fw.z, dk * fw.w);
-            const double t = fmax(0.0, 1.0 - fabs(dx)) * fmax(0.0, 1.0 - fabs(dy));
+            const double t = tent_q23(dx) * tent_q23(dy);
             w[sb + 1] += kvalid ? t : 0.0;
         }
     }

@@ -105,3 +105,35 @@ def test_default_mask_counts():
     """Q2 mask; in-FOV voxel counts quoted in SURVEY.md 8 table (3 024 for C1, 99 936 for C2)."""
     assert int(Oracle(ki.config("C1")).default_mask().sum()) == 3024
     assert int(Oracle(ki.config("C2")).default_mask().sum()) * 8 == 99936
+
+
+def test_q23_samples_on_pixel_centres_leave_no_residue_on_the_neighbours():
+    """Reading Q23.  At 0 and 90 degrees with bin = step = voxel every sample of P2 lies exactly on a pixel centre, so in
+    exact arithmetic one sinogram bin back-projects onto ONE image column (row) and nothing else.  With the mMR voxel size
+    2.09 mm the index fx = X / vx + (nx - 1)/2 carries ~1e-14 of rounding for some bins (b = 48 of 344 is one); without the
+    snap that leaves a weight of 1.4e-14 on the neighbouring column, which a noise-dominated OSL update amplifies by 20
+    orders of magnitude within one pass (Q23).  Pin (C4's in-plane geometry): the back-projection of
+    ANY single bin at those two angles is exactly step_mm on its column / row and EXACTLY zero everywhere else; the
+    brute-force tent matrix (test_brute_force_matrix_tiny) still matches to 1e-12, i.e. the snap moves no weight by more
+    than 1e-9."""
+    n, A = 344, 252
+    cfg = ki.small_config(nx=n, ny=n, n_angles=A, n_bins=n, n_subsets=21, n_steps=n, vx=2.09, vy=2.09, bin_mm=2.09, step_mm=2.09)
+    o = Oracle(cfg)
+    bins = [3, 46, 47, 48, 171, 172, 300, 343]
+    for a, axis in ((0, "column"), (A // 2, "row")):
+        q = np.zeros((len(bins), 1, A, n))           # "frame" f holds the unit sinogram of bin bins[f]
+        q[np.arange(len(bins)), 0, a, bins] = 1.0
+        img = o.back_project(q)[:, 0]                # [f][ny][nx]
+        for f, b in enumerate(bins):
+            want = np.zeros((n, n))
+            if axis == "column":
+                want[:, b] = cfg["step_mm"]          # theta = 0: X = s_b, the ray runs along y through column b
+            else:
+                want[b, :] = cfg["step_mm"]          # theta = 90 degrees: Y = s_b, the ray runs along x through row b
+            assert np.count_nonzero(img[f]) == n, (a, b, np.count_nonzero(img[f]))
+            assert np.array_equal(img[f], want), (a, b)
+    # forward: the same columns / rows (sums of n pixels times step)
+    x = np.random.default_rng(5).random((1, 1, n, n))
+    y = o.forward_project(x)[0, 0]
+    np.testing.assert_allclose(y[0], cfg["step_mm"] * x[0, 0].sum(axis=0), rtol=1e-13)
+    np.testing.assert_allclose(y[A // 2], cfg["step_mm"] * x[0, 0].sum(axis=1), rtol=1e-13)
