@@ -128,19 +128,24 @@ int ensure_border(kcs_ctx *c, int Tp) {
     return KCS_OK;
 }
 
-int pack_image(kcs_ctx *c, const float *planar, int nf, float *inner, int Tp) {
+// slices [z0, z0 + nzc) of a planar image [nf][nz][ny][nx]  <->  the padded frame-innermost layout
+int pack_image(kcs_ctx *c, const float *planar, int nf, float *inner, int Tp, int z0 = 0, int nzc = -1) {
     const KGeom &g = c->g;
-    return kcs_launch_pack(c, planar, c->n_vox, nf, inner, Tp, (long long)g.nz * g.ny, g.nx, g.ny,
-                           (long long)g.nyp * g.nxp, g.nxp, KCS_PAD * (g.nxp + 1));
+    if (nzc < 0) nzc = g.nz;
+    return kcs_launch_pack(c, planar + (size_t)z0 * g.ny * g.nx, c->n_vox, nf, inner + (size_t)z0 * g.nyp * g.nxp * Tp, Tp,
+                           (long long)nzc * g.ny, g.nx, g.ny, (long long)g.nyp * g.nxp, g.nxp, KCS_PAD * (g.nxp + 1));
 }
-int unpack_image(kcs_ctx *c, const float *inner, int Tp, float *planar, int nf) {
+int unpack_image(kcs_ctx *c, const float *inner, int Tp, float *planar, int nf, int z0 = 0, int nzc = -1) {
     const KGeom &g = c->g;
-    return kcs_launch_unpack(c, inner, Tp, planar, c->n_vox, nf, (long long)g.nz * g.ny, g.nx, g.ny,
-                             (long long)g.nyp * g.nxp, g.nxp, KCS_PAD * (g.nxp + 1));
+    if (nzc < 0) nzc = g.nz;
+    return kcs_launch_unpack(c, inner + (size_t)z0 * g.nyp * g.nxp * Tp, Tp, planar + (size_t)z0 * g.ny * g.nx, c->n_vox, nf,
+                             (long long)nzc * g.ny, g.nx, g.ny, (long long)g.nyp * g.nxp, g.nxp, KCS_PAD * (g.nxp + 1));
 }
-int pack_sino(kcs_ctx *c, const float *planar, int nf, float *inner, int Tp, int As) {
+int pack_sino(kcs_ctx *c, const float *planar, int nf, float *inner, int Tp, int As, int z0 = 0, int nzc = -1) {
     const KGeom &g = c->g;
-    return kcs_launch_pack(c, planar, (size_t)g.nz * As * g.B, nf, inner, Tp, (long long)g.nz * As, g.B, INT_MAX, 0, g.B, 0);
+    if (nzc < 0) nzc = g.nz;
+    return kcs_launch_pack(c, planar + (size_t)z0 * As * g.B, (size_t)g.nz * As * g.B, nf, inner + (size_t)z0 * As * g.B * Tp, Tp,
+                           (long long)nzc * As, g.B, INT_MAX, 0, g.B, 0);
 }
 int unpack_sino(kcs_ctx *c, const float *inner, int Tp, float *planar, int nf, int As) {
     const KGeom &g = c->g;
@@ -208,8 +213,9 @@ int kcs_destroy(kcs_ctx *c) {
         if (p) cudaFree(p);
     for (const KProfRec &r : c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
-    if (c->ev_x) cudaEventDestroy(c->ev_x);
-    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->in_stream) { cudaStreamDestroy(c->in_stream); cudaStreamDestroy(c->out_stream); cudaEventDestroy(c->ev_small); }
+    for (cudaEvent_t e : c->ev_in) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->ev_out) cudaEventDestroy(e);
     if (c->aux_stream) { cudaStreamDestroy(c->aux_stream); cudaEventDestroy(c->ev_fork); cudaEventDestroy(c->ev_join); }
     delete c;
     return KCS_OK;
@@ -246,7 +252,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->xi = c->Fi = c->qi = c->yi = c->ri = c->r_pad = c->theta2 = nullptr;
     c->thD[0] = c->thD[1] = c->lamD = nullptr;
     c->lm_state = nullptr;
-    c->ev_x = nullptr; c->copy_stream = nullptr;
+    c->in_stream = c->out_stream = nullptr; c->ev_small = nullptr;
     c->aux_stream = nullptr; c->ev_fork = c->ev_join = nullptr;
     c->st_y = c->st_r = c->st_x = c->st_theta = c->st_lambda = nullptr;
     c->st_r_elems = 0;
@@ -397,7 +403,7 @@ int kcs_forward_project(kcs_ctx *c, const float *x, float *y_s, int subset, int 
     const int Tp = round_up4(nf), As = subset < 0 ? g.A : g.A / g.S;
     if ((rc = ensure_border(c, Tp))) return rc;
     if ((rc = pack_image(c, x + (size_t)f0 * c->n_vox, nf, c->xi, Tp))) return rc;
-    if ((rc = kcs_launch_forward(c, Tp, subset, 0, 1.f, 0, 0))) return rc;
+    if ((rc = kcs_launch_forward(c, Tp, subset, 0, 1.f, 0, 0, 0, g.nz))) return rc;
     return unpack_sino(c, c->qi, Tp, y_s + (size_t)f0 * g.nz * As * g.B, nf, As);
 }
 
@@ -410,7 +416,7 @@ int kcs_back_project(kcs_ctx *c, const float *q_s, float *b, int subset, int f0,
     const int Tp = round_up4(nf), As = subset < 0 ? g.A : g.A / g.S;
     if ((rc = ensure_border(c, Tp))) return rc;
     if ((rc = pack_sino(c, q_s + (size_t)f0 * g.nz * As * g.B, nf, c->qi, Tp, As))) return rc;
-    if ((rc = kcs_launch_back(c, Tp, subset, 0, c->xi, 1.f, 0.f))) return rc;
+    if ((rc = kcs_launch_back(c, Tp, subset, 0, c->xi, 1.f, 0.f, 0, g.nz))) return rc;
     return unpack_image(c, c->xi, Tp, b + (size_t)f0 * c->n_vox, nf);
 }
 
@@ -492,22 +498,36 @@ static int start_kinetic(kcs_ctx *c, const float *theta, int Tp) {
     return KCS_OK;
 }
 
-// x_final (may be NULL): recorded on the context's stream as soon as the caller's x holds its final value, i.e. before
-// the last MAP-LM -- kcs_icm_run_host starts the device-to-host copy of x there, on a second stream, behind the fit.
+// Host-buffer mode of the ICM loop (kcs_icm_run_host): y and x arrive from / x returns to HOST memory in z chunks.
+struct HostIO {
+    const float *hy;   // [host] y[T][nz][A][B]
+    float *hx;         // [host] x[T][nz][ny][nx], in and out
+    int nchunk;
+};
+
+static void chunk_range(const KGeom &g, int nchunk, int k, int &z0, int &nzc) {
+    const int per = (g.nz + nchunk - 1) / nchunk;
+    z0 = k * per;
+    nzc = z0 >= g.nz ? 0 : (z0 + per > g.nz ? g.nz - z0 : per);
+}
+
+// The ICM loop.  y, x: DEVICE buffers (the caller's, or the staging buffers of kcs_icm_run_host when io != NULL).
+// The OS pass runs chunk by chunk in z (direct planes are independent, so the result does not depend on the chunking);
+// with io, chunk k's inputs are awaited just before its first kernel and its final x is handed to the copy-out stream
+// right after its last OSL update of the last iteration.
 static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta,
                         float *lambda, float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter,
-                        cudaEvent_t x_final) {
+                        const HostIO *io) {
     if (!c) return KCS_ERR_NULL;
     if (!y || !r || !x || !theta || !lambda) return fail(c, KCS_ERR_NULL, "kcs_icm: NULL buffer");
     if (r_mode != KCS_R_PER_FRAME && r_mode != KCS_R_FULL) return fail(c, KCS_ERR_SHAPE, "kcs_icm: unknown r_mode");
     if (n_lm < 0 || n_iter < 0 || !(scale > 0.f)) return fail(c, KCS_ERR_SHAPE, "kcs_icm: bad n_lm / n_iter / scale");
     const KGeom &g = c->g;
     const int T = c->cfg.n_frames, Tp = round_up4(T);
+    const int nchunk = io ? io->nchunk : 1;
     int rc;
     if (n_iter > 0 && (rc = start_kinetic(c, theta, Tp))) return rc;  // beside the packing and the first forward projection
     if ((rc = ensure_border(c, Tp))) return rc;
-    if ((rc = pack_image(c, x, T, c->xi, Tp))) return rc;
-    if ((rc = pack_sino(c, y, T, c->yi, Tp, g.A))) return rc;
     if (r_mode == KCS_R_PER_FRAME) {
         KCS_CUDA_OK(c, cudaMemsetAsync(c->r_pad, 0, KCS_MAX_FRAMES * sizeof(float), c->stream));
         KCS_CUDA_OK(c, cudaMemcpyAsync(c->r_pad, r, T * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
@@ -520,17 +540,35 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
         }
         if ((rc = pack_sino(c, r, T, c->ri, Tp, g.A))) return rc;
     }
+    if (n_iter == 0 || !io) {  // device-resident call: pack everything up front (one chunk)
+        if ((rc = pack_image(c, x, T, c->xi, Tp))) return rc;
+        if ((rc = pack_sino(c, y, T, c->yi, Tp, g.A))) return rc;
+    }
     for (int it = 0; it < n_iter; ++it) {
         const float b = it == 0 ? beta_first : beta;
-        if (it > 0 && (rc = start_kinetic(c, theta, Tp))) return rc;
-        for (int s = 0; s < g.S; ++s) {  // Q5: subsets in order 0..S-1
-            // after the first OSL update of this call x is zero outside the mask: rays are clipped to the FOV circle
-            if ((rc = kcs_launch_forward(c, Tp, s, 1, scale, r_mode, (it > 0 || s > 0) ? 1 : 0))) return rc;
-            if (s == 0) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
-            if ((rc = kcs_launch_back(c, Tp, s, 1, nullptr, scale, b))) return rc;
-        }
         const bool last = it == n_iter - 1;
-        if (last) {  // the activity is final after the last OS pass; MAP-LM only reads it: unpack beside the fit
+        if (it > 0 && (rc = start_kinetic(c, theta, Tp))) return rc;
+        for (int k = 0; k < nchunk; ++k) {
+            int z0, nzc;
+            chunk_range(g, nchunk, k, z0, nzc);
+            if (nzc == 0) continue;
+            if (io && it == 0) {  // this chunk's x and y have been copied to the staging buffers: pack them
+                KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_in[k], 0));
+                if ((rc = pack_image(c, x, T, c->xi, Tp, z0, nzc))) return rc;
+                if ((rc = pack_sino(c, y, T, c->yi, Tp, g.A, z0, nzc))) return rc;
+            }
+            for (int s = 0; s < g.S; ++s) {  // Q5: subsets in order 0..S-1
+                // after the first OSL update of this call x is zero outside the mask: rays are clipped to the FOV circle
+                if ((rc = kcs_launch_forward(c, Tp, s, 1, scale, r_mode, (it > 0 || s > 0) ? 1 : 0, z0, nzc))) return rc;
+                if (s == 0 && k == 0) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
+                if ((rc = kcs_launch_back(c, Tp, s, 1, nullptr, scale, b, z0, nzc))) return rc;
+            }
+            if (io && last) {  // this chunk's activity is final: unpack it and let the copy-out stream take it
+                if ((rc = unpack_image(c, c->xi, Tp, x, T, z0, nzc))) return rc;
+                KCS_CUDA_OK(c, cudaEventRecord(c->ev_out[k], c->stream));
+            }
+        }
+        if (last && !io) {  // the activity is final after the last OS pass; MAP-LM only reads it: unpack beside the fit
             cudaStream_t main_stream = c->stream;
             KCS_CUDA_OK(c, cudaEventRecord(c->ev_fork, main_stream));
             KCS_CUDA_OK(c, cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
@@ -539,14 +577,12 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
             c->stream = main_stream;
             if (rc) return rc;
             KCS_CUDA_OK(c, cudaEventRecord(c->ev_join, c->aux_stream));
-            if (x_final) KCS_CUDA_OK(c, cudaEventRecord(x_final, c->aux_stream));
         }
         if ((rc = lm_steps(c, c->xi, 1, Tp, theta, lambda, gamma, delta, n_lm, nullptr))) return rc;
-        if (last) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
+        if (last && !io) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
     }
     if (n_iter == 0) {
         if ((rc = unpack_image(c, c->xi, Tp, x, T))) return rc;
-        if (x_final) KCS_CUDA_OK(c, cudaEventRecord(x_final, c->stream));
     }
     return KCS_OK;
 }
@@ -566,6 +602,7 @@ int kcs_icm_run_host(kcs_ctx *c, const float *y, const float *r, int r_mode, flo
     if (!c) return KCS_ERR_NULL;
     if (!y || !r || !x || !theta || !lambda) return fail(c, KCS_ERR_NULL, "kcs_icm_run_host: NULL buffer");
     if (r_mode != KCS_R_PER_FRAME && r_mode != KCS_R_FULL) return fail(c, KCS_ERR_SHAPE, "kcs_icm_run_host: unknown r_mode");
+    const KGeom &g = c->g;
     const int T = c->cfg.n_frames;
     const size_t ny_ = (size_t)T * c->n_ray_all, nx_ = (size_t)T * c->n_vox;
     const size_t nr = r_mode == KCS_R_PER_FRAME ? (size_t)T : ny_;
@@ -586,26 +623,65 @@ int kcs_icm_run_host(kcs_ctx *c, const float *y, const float *r, int r_mode, flo
         cudaGetLastError();
         return fail(c, KCS_ERR_ALLOC, std::string("kcs_icm_run_host: ") + cudaGetErrorString(e));
     }
-    cudaStream_t st = c->stream;
-    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_y, y, ny_ * sizeof(float), cudaMemcpyHostToDevice, st));
-    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_r, r, nr * sizeof(float), cudaMemcpyHostToDevice, st));
-    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_x, x, nx_ * sizeof(float), cudaMemcpyHostToDevice, st));
-    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_theta, theta, 4 * c->n_vox * sizeof(float), cudaMemcpyHostToDevice, st));
-    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_lambda, lambda, c->n_vox * sizeof(float), cudaMemcpyHostToDevice, st));
-    if (!c->ev_x) {
-        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_x, cudaEventDisableTiming));
-        KCS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    // z chunks of >= 16 slices, at most 8 of them: big enough to fill the GPU, small enough to hide the copies
+    HostIO io{y, x, g.nz / 16 < 1 ? 1 : (g.nz / 16 > 8 ? 8 : g.nz / 16)};
+    if (!c->in_stream) {
+        KCS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->in_stream, cudaStreamNonBlocking));
+        KCS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->out_stream, cudaStreamNonBlocking));
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_small, cudaEventDisableTiming));
     }
+    while ((int)c->ev_in.size() < io.nchunk) {
+        cudaEvent_t a = nullptr, b = nullptr;
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+        c->ev_in.push_back(a);
+        c->ev_out.push_back(b);
+    }
+    cudaStream_t st = c->stream, in = c->in_stream, out = c->out_stream;
+    // the copy-in stream starts behind whatever the caller has enqueued on the context's stream (the staging buffers
+    // may still be in use by a previous call)
+    KCS_CUDA_OK(c, cudaEventRecord(c->ev_small, st));
+    KCS_CUDA_OK(c, cudaStreamWaitEvent(in, c->ev_small, 0));
+    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_theta, theta, 4 * c->n_vox * sizeof(float), cudaMemcpyHostToDevice, in));
+    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_lambda, lambda, c->n_vox * sizeof(float), cudaMemcpyHostToDevice, in));
+    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_r, r, nr * sizeof(float), cudaMemcpyHostToDevice, in));
+    KCS_CUDA_OK(c, cudaEventRecord(c->ev_small, in));
+    for (int k = 0; k < io.nchunk; ++k) {  // x and y of chunk k: T strided pieces each (one 2-D copy)
+        int z0, nzc;
+        chunk_range(g, io.nchunk, k, z0, nzc);
+        if (nzc > 0) {
+            const size_t v2 = (size_t)g.ny * g.nx, r2 = (size_t)g.A * g.B;
+            KCS_CUDA_OK(c, cudaMemcpy2DAsync(c->st_x + z0 * v2, c->n_vox * sizeof(float), x + z0 * v2, c->n_vox * sizeof(float),
+                                             nzc * v2 * sizeof(float), T, cudaMemcpyHostToDevice, in));
+            KCS_CUDA_OK(c, cudaMemcpy2DAsync(c->st_y + z0 * r2, c->n_ray_all * sizeof(float), y + z0 * r2,
+                                             c->n_ray_all * sizeof(float), nzc * r2 * sizeof(float), T, cudaMemcpyHostToDevice, in));
+        }
+        KCS_CUDA_OK(c, cudaEventRecord(c->ev_in[k], in));
+    }
+    KCS_CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_small, 0));
+    if (n_iter <= 0)  // nothing to overlap: wait for every chunk, the loop below only unpacks
+        for (int k = 0; k < io.nchunk; ++k) KCS_CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_in[k], 0));
     int rc = icm_run_impl(c, c->st_y, c->st_r, r_mode, scale, c->st_x, c->st_theta, c->st_lambda, beta_first, beta, gamma, delta,
-                          n_lm, n_iter, c->ev_x);
+                          n_lm, n_iter, n_iter > 0 ? &io : nullptr);
     if (rc) return rc;
-    // x goes back on a second stream while the last MAP-LM still runs on the first
-    KCS_CUDA_OK(c, cudaStreamWaitEvent(c->copy_stream, c->ev_x, 0));
-    KCS_CUDA_OK(c, cudaMemcpyAsync(x, c->st_x, nx_ * sizeof(float), cudaMemcpyDeviceToHost, c->copy_stream));
+    if (n_iter > 0) {
+        for (int k = 0; k < io.nchunk; ++k) {  // x of chunk k goes back while later chunks and the last MAP-LM still run
+            int z0, nzc;
+            chunk_range(g, io.nchunk, k, z0, nzc);
+            if (nzc == 0) continue;
+            const size_t v2 = (size_t)g.ny * g.nx;
+            KCS_CUDA_OK(c, cudaStreamWaitEvent(out, c->ev_out[k], 0));
+            KCS_CUDA_OK(c, cudaMemcpy2DAsync(x + z0 * v2, c->n_vox * sizeof(float), c->st_x + z0 * v2, c->n_vox * sizeof(float),
+                                             nzc * v2 * sizeof(float), T, cudaMemcpyDeviceToHost, out));
+        }
+    } else {
+        KCS_CUDA_OK(c, cudaMemcpyAsync(x, c->st_x, nx_ * sizeof(float), cudaMemcpyDeviceToHost, st));
+    }
     KCS_CUDA_OK(c, cudaMemcpyAsync(theta, c->st_theta, 4 * c->n_vox * sizeof(float), cudaMemcpyDeviceToHost, st));
     KCS_CUDA_OK(c, cudaMemcpyAsync(lambda, c->st_lambda, c->n_vox * sizeof(float), cudaMemcpyDeviceToHost, st));
     KCS_CUDA_OK(c, cudaStreamSynchronize(st));
-    KCS_CUDA_OK(c, cudaStreamSynchronize(c->copy_stream));
+    KCS_CUDA_OK(c, cudaStreamSynchronize(out));
+    KCS_CUDA_OK(c, cudaStreamSynchronize(in));
     return KCS_OK;
 }
 

@@ -107,10 +107,13 @@ struct kcs_ctx {
     // device staging buffers of kcs_icm_run_host, allocated lazily
     float *st_y, *st_r, *st_x, *st_theta, *st_lambda;
     size_t st_r_elems;
-    cudaEvent_t ev_x;          // kcs_icm_run_host: x is final (recorded before the last MAP-LM)
     cudaStream_t aux_stream;   // kcs_icm_run: the kinetic evaluator runs here beside the first forward projection
     cudaEvent_t ev_fork, ev_join;
-    cudaStream_t copy_stream;  // kcs_icm_run_host: device-to-host copy of x behind the last MAP-LM
+    // kcs_icm_run_host: the volume moves in z chunks; chunk k + 1 is copied in (in_stream) and chunk k - 1 copied out
+    // (out_stream) while chunk k goes through its OS pass on the context's stream
+    cudaStream_t in_stream, out_stream;
+    cudaEvent_t ev_small;                  // theta, lambda, r are on the device
+    std::vector<cudaEvent_t> ev_in, ev_out;  // per chunk: inputs have arrived / x is final on the device
 };
 
 #define KCS_CUDA_OK(ctx, call)                                                                  \
@@ -160,14 +163,14 @@ int kcs_launch_pack(kcs_ctx *c, const float *src, size_t fs, int nf, float *dst,
                     int rps, long long slab, int rstride, int off);
 int kcs_launch_unpack(kcs_ctx *c, const float *src, int Tp, float *dst, size_t fs, int nf, long long nrows, int W,
                       int rps, long long slab, int rstride, int off);
-// forward projection of c->xi (Tp frames) for `subset`; out = c->qi.
+// forward projection of slices [z0, z0 + nzc) of c->xi (Tp frames) for `subset`; out = c->qi.
 //   ratio == 0:  qi = step * sum                      (kcs_forward_project)
 //   ratio == 1:  qi = y / (scale*step*sum + r), 0 where the denominator <= 1e-12   (O1)
-int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, int r_mode, int clip_fov);
-// gather back-projection of c->qi for `subset`.
+int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, int r_mode, int clip_fov, int z0, int nzc);
+// gather back-projection of slices [z0, z0 + nzc) of c->qi for `subset`.
 //   osl == 0:  out_inner (padded layout) = step * sum                              (kcs_back_project)
 //   osl == 1:  c->xi <- OSL update with bp = scale*step*sum, sens = scale*A_s^T 1, F = c->Fi   (O2)
-int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, float scale, float beta);
+int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, float scale, float beta, int z0, int nzc);
 int kcs_launch_sens(kcs_ctx *c);  // fills d_sens, d_smax
 int kcs_launch_build_wtab(kcs_ctx *c);  // fills d_wtab
 int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *sens, const float *F, float beta,

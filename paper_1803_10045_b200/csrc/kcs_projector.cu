@@ -252,14 +252,20 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, 1) k_forward(KGeom g, FwdArgs p) 
     }
 }
 
-int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, int r_mode, int clip_fov) {
-    const KGeom &g = c->g;
+int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, int r_mode, int clip_fov, int z0, int nzc) {
+    KGeom g = c->g;
+    if (nzc <= 0) return KCS_OK;
+    g.nz = nzc;  // slices [z0, z0 + nzc): direct planes are independent, a z range is a smaller problem of the same kind
     FwdArgs p;
-    p.xi = c->xi; p.qi = c->qi; p.yi = c->yi; p.ri = c->ri; p.r_pad = c->r_pad;
     p.Tp = Tp;
     const int FPT = 4;  // one LDG.128 per lane and tap
     p.FG = Tp / FPT;
     p.As = subset < 0 ? g.A : g.A / g.S;
+    p.xi = c->xi + (size_t)z0 * g.nyp * g.nxp * Tp;
+    p.qi = c->qi + (size_t)z0 * p.As * g.B * Tp;
+    p.yi = c->yi + (size_t)z0 * g.A * g.B * Tp;
+    p.ri = c->ri ? c->ri + (size_t)z0 * g.A * g.B * Tp : nullptr;
+    p.r_pad = c->r_pad;
     p.subset = subset;
     p.ratio = ratio; p.r_mode = r_mode; p.scale = scale;
     p.clip_r2 = clip_fov ? c->fov_rc2 : -1.f;
@@ -572,12 +578,15 @@ __global__ void __launch_bounds__(256, 2) k_back(KGeom g, BackArgs p) {
     }
 }
 
-int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, float scale, float beta) {
-    const KGeom &g = c->g;
+int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, float scale, float beta, int z0, int nzc) {
+    KGeom g = c->g;
+    if (nzc <= 0) return KCS_OK;
+    g.nz = nzc;  // slices [z0, z0 + nzc)
     BackArgs p;
-    p.qi = c->qi;
-    p.out = osl ? c->xi : out_inner;
-    p.Fi = c->Fi;
+    const size_t zpix = (size_t)z0 * g.nyp * g.nxp * Tp;
+    p.qi = c->qi + (size_t)z0 * (subset < 0 ? g.A : g.A / g.S) * g.B * Tp;
+    p.out = (osl ? c->xi : out_inner) + zpix;
+    p.Fi = c->Fi + zpix;
     const int sidx = subset < 0 ? g.S : subset;
     p.sens = c->d_sens + (size_t)sidx * g.nx * g.ny;
     p.smax = c->d_smax + sidx;

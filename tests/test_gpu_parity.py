@@ -382,6 +382,35 @@ def test_icm_10_iterations(name):
     ctx.close()
 
 
+def test_host_entry_moves_the_volume_in_z_chunks():
+    """kcs_icm_run_host copies x and y in z chunks (>= 16 slices each) while earlier chunks go through their OS pass, and
+    returns x chunk by chunk; direct planes are independent, so the result must equal kcs_icm_run bit for bit -- for one
+    iteration (copy-in and copy-out chunked in the same pass) and for three."""
+    cfg = ki.small_config(nx=24, ny=20, nz=37, n_angles=12, n_bins=24, n_subsets=3, counts=4e5)
+    o = Oracle(cfg)
+    ctx = _kcs().Context(cfg)
+    mask = o.default_mask()
+    prob = ki.make_problem(cfg, mask, o.kinetic_eval, o.forward_project, noisy=True)
+    x0, th0, lam0 = ki.initial_state(cfg, mask, prob["y"], prob["r"], prob["scale"], o.forward_project)
+    y, rd, scale = dev(prob["y"]), dev(prob["r"]), float(prob["scale"])
+    for n_iter in (1, 3):
+        x, th, lam = dev(x0), dev(th0), dev(lam0)
+        ctx.icm_run(y, rd, scale, x, th, lam, 0.0, cfg["beta"], cfg["gamma"], cfg["delta"], 2, n_iter)
+        hx, hth, hlam = np.float32(x0), np.float32(th0), np.float32(lam0)
+        ctx.icm_run_host(np.float32(prob["y"]), np.float32(prob["r"]), scale, hx, hth, hlam, 0.0, cfg["beta"], cfg["gamma"],
+                         cfg["delta"], 2, n_iter)
+        assert np.array_equal(hx, x.cpu().numpy()) and np.array_equal(hth, th.cpu().numpy())
+        assert np.array_equal(hlam, lam.cpu().numpy())
+    # full randoms sinogram and pinned buffers take the same path
+    rfull = np.ascontiguousarray(np.broadcast_to(np.float32(prob["r"])[:, None, None, None], prob["y"].shape))
+    px = torch.tensor(np.float32(x0)).pin_memory(); pth = torch.tensor(np.float32(th0)).pin_memory()
+    plam = torch.tensor(np.float32(lam0)).pin_memory()
+    ctx.icm_run_host(torch.tensor(np.float32(prob["y"])).pin_memory(), torch.tensor(rfull).pin_memory(), scale, px, pth, plam,
+                     0.0, cfg["beta"], cfg["gamma"], cfg["delta"], 2, 3)
+    assert np.array_equal(px.numpy(), hx) and np.array_equal(pth.numpy(), hth)
+    ctx.close()
+
+
 def test_projector_C2_full_size():
     """C2 geometry (128x128x8, 120x128, T = 24): several blocks per slice and z-batching in the back-projector."""
     cfg = CONFIGS["C2"]()
