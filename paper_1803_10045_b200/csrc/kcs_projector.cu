@@ -274,8 +274,10 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
         while ((1 << ib) < (g.nxp > g.nyp ? g.nxp : g.nyp) + 2 * KCS_ANCHOR) ++ib;
         p.FB = 31 - ib > 22 ? 22 : 31 - ib;
     }
-    // parallelism: split the K steps of a ray over KSPLIT threads when there are too few rays to fill 148 SMs
-    const long long base = (long long)g.nz * p.As * g.B * p.FG;
+    // parallelism: split the K steps of a ray over KSPLIT threads when there are too few rays to fill 148 SMs.  Decided on
+    // the WHOLE volume, not on the z range of this launch: the split fixes the order of a ray's partial sums, and a chunked
+    // pass (kcs_icm_run_host) must reproduce the unchunked one bit for bit.
+    const long long base = (long long)c->g.nz * p.As * g.B * p.FG;
     int ks = 1;
     while (base * ks < 148LL * 2048 && ks < 8 && g.K / (ks * 2) >= 16) ks *= 2;
     p.KSPLIT = ks;

@@ -386,7 +386,9 @@ def test_host_entry_moves_the_volume_in_z_chunks():
     """kcs_icm_run_host copies x and y in z chunks (>= 16 slices each) while earlier chunks go through their OS pass, and
     returns x chunk by chunk; direct planes are independent, so the result must equal kcs_icm_run bit for bit -- for one
     iteration (copy-in and copy-out chunked in the same pass) and for three."""
-    cfg = ki.small_config(nx=24, ny=20, nz=37, n_angles=12, n_bins=24, n_subsets=3, counts=4e5)
+    # 96 x 96 x 64, T = 29: the whole volume is past the forward projector's K-split threshold (148 x 2048 ray lanes), one
+    # of its four 16-slice chunks alone is not -- the split must be decided on the whole volume
+    cfg = ki.small_config(nx=96, ny=96, nz=64, n_angles=24, n_bins=96, n_subsets=3, counts=4e6, sched="C3")
     o = Oracle(cfg)
     ctx = _kcs().Context(cfg)
     mask = o.default_mask()
