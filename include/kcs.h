@@ -17,6 +17,7 @@
  *        sinogram   y[T][nz][A][B]            subset sinogram  y_s[T][nz][A/S][B]  (local angle la <-> a = s + la*S)
  *        maps       theta[4][nz][ny][nx]      parameter order (K1, k2, k3, vB)
  *        lambda, cost [nz][ny][nx]
+ *     (with kcs_config.n_replicas = N > 1 read N*nz for nz everywhere below)
  *   - Internally the hot path keeps activity and sinograms frame-innermost ([voxel][Tp], Tp = the power
  *     of two >= T, 4..32) so that one cache line fetched for a bilinear tap serves every time frame
  *     (BJ north_star); the pack/unpack transposes are part of the calls below.
@@ -61,6 +62,11 @@ typedef struct {
     float feng_A[3];                /* BJ configs[0](1): Cp(t) = (A1 t - A2 - A3) e^{-l1 t} + A2 e^{-l2 t} + A3 e^{-l3 t} */
     float feng_lambda[3];
     const unsigned char *mask_host; /* [host][ny][nx] field-of-view mask, NULL = Q2 default disc */
+    int n_replicas;                 /* N >= 1 (0 is read as 1): noise realisations of one object reconstructed in one
+                                     * batch ("100 noisy realizations").  They share geometry, sensitivity, weight
+                                     * table and kinetic tables; every buffer then carries N * nz slices, replica-major
+                                     * (slice index = replica * nz + z), e.g. x[T][N*nz][ny][nx].  Replicas never interact:
+                                     * the 6-neighbourhood of the Huber prior stops at a replica's first and last slice. */
 } kcs_config;
 
 /* Create / destroy.  `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
@@ -127,6 +133,10 @@ int kcs_kinetic_eval(kcs_ctx *ctx, const float *theta, float *F, float *J);
  * receives Phi_v after the last step.  Out-of-mask voxels are left untouched (cost 0). */
 int kcs_map_lm(kcs_ctx *ctx, const float *x, float *theta, float *lambda, float gamma, float delta,
                int n_steps, float *cost);
+
+/* the macro-parameter map K_i = K1 k3 / (k2 + k3) (net influx rate; 0 where k2 + k3 = 0) from
+ * theta[4][nz][ny][nx]; ki[nz][ny][nx] (device).  Evaluated for every voxel. */
+int kcs_ki_map(kcs_ctx *ctx, const float *theta, float *ki);
 
 /* I: one ICM iteration,
  *   F <- K(theta);  for s = 0..S-1: yhat = scale A_s x + r, q = y/yhat (0 where yhat <= 1e-12),

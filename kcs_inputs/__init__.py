@@ -173,6 +173,17 @@ def poisson(mean: np.ndarray, seed: int) -> np.ndarray:
     return rng.poisson(np.maximum(mean, 0.0)).astype(np.float64)
 
 
+def noise_realisations(ybar: np.ndarray, seed: int, n: int) -> np.ndarray:
+    """P:131 ("100 noisy realizations"): n independent Poisson draws of one noise-free sinogram ybar[T,nz,A,B], stacked
+    replica-major along z -> [T, n*nz, A, B].  Realisation k uses PCG64(seed + 1000 + k), so realisation 0 is `poisson`."""
+    return np.concatenate([poisson(ybar, seed + k) for k in range(n)], axis=1)
+
+
+def tile_replicas(a: np.ndarray, axis: int, n: int) -> np.ndarray:
+    """The same array for every replica, replica-major along the slice axis."""
+    return np.concatenate([a] * n, axis=axis)
+
+
 def lm_start(theta_true: np.ndarray, seed: int) -> np.ndarray:
     """C5(b): initial parameters uniform within +/-50 % of the truth."""
     rng = np.random.Generator(np.random.PCG64(seed))

@@ -244,6 +244,32 @@ class Oracle:
         return (x.reshape(self.T, self.nz, self.ny, self.nx),
                 theta.reshape(4, self.nz, self.ny, self.nx), lam.reshape(self.nz, self.ny, self.nx))
 
+    def icm_iteration_replicas(self, n_replicas, y, r, scale, x, theta, lam, beta, gamma, delta, n_lm):
+        """N noise realisations of one object are N independent reconstructions.  Buffers are replica-major along z
+        ([.., N*nz, ..]); this simply runs `icm_iteration` on each replica's slices in turn."""
+        nz = self.nz
+        y, x, theta, lam = _f64(y), _f64(x), _f64(theta), _f64(lam)
+        y = y.reshape(self.T, n_replicas * nz, self.A, self.B)
+        x = x.reshape(self.T, n_replicas * nz, self.ny, self.nx)
+        theta = theta.reshape(4, n_replicas * nz, self.ny, self.nx)
+        lam = lam.reshape(n_replicas * nz, self.ny, self.nx)
+        xs, ths, lams = [], [], []
+        for k in range(n_replicas):
+            sl = slice(k * nz, (k + 1) * nz)
+            a, b, c = self.icm_iteration(np.ascontiguousarray(y[:, sl]), r, scale, np.ascontiguousarray(x[:, sl]),
+                                         np.ascontiguousarray(theta[:, sl]), np.ascontiguousarray(lam[sl]), beta, gamma, delta, n_lm)
+            xs.append(a); ths.append(b); lams.append(c)
+        return np.concatenate(xs, axis=1), np.concatenate(ths, axis=1), np.concatenate(lams, axis=0)
+
+    @staticmethod
+    def ki_map(theta):
+        """K_i = K1 k3 / (k2 + k3)."""
+        theta = _f64(theta)
+        V = theta.size // 4
+        ki = np.zeros(V)
+        _L().kcso_ki_map(_p(theta), _p(ki), C.c_long(V))
+        return ki.reshape(theta.shape[1:])
+
     def poisson_loglik(self, y, r, scale, x) -> float:
         y, x = _f64(y), _f64(x)
         r, mode = self._r(r)

@@ -686,3 +686,11 @@ double kcso_poisson_loglik(const kcso_config *c, const double *y, const double *
     free(yh);
     return ll;
 }
+
+/* K_i = K1 k3 / (k2 + k3), the net influx rate (S8c-K2: B2 = K1 k3 / a "= K_i"); 0 where k2 + k3 = 0. theta[4][V]. */
+void kcso_ki_map(const double *theta, double *ki, long V) {
+    for (long v = 0; v < V; ++v) {
+        const double K1 = theta[v], k2 = theta[V + v], k3 = theta[2 * V + v];
+        ki[v] = (k2 + k3 > 0.0) ? K1 * k3 / (k2 + k3) : 0.0;
+    }
+}

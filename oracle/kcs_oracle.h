@@ -94,6 +94,9 @@ void kcso_os_pass(const kcso_config *c, const double *y, const double *r, int r_
 void kcso_icm_iteration(const kcso_config *c, const double *y, const double *r, int r_mode, double scale,
                         double *x, double *theta, double *lambda,
                         double beta, double gamma, double delta, int n_lm);
+/* K_i = K1 k3 / (k2 + k3) for V voxels, theta[4][V]; 0 where k2 + k3 = 0. */
+void kcso_ki_map(const double *theta, double *ki, long V);
+
 /* Poisson log-likelihood sum(y log yhat - yhat), yhat = scale A x + r, all angles (eq. 1 without the prior). */
 double kcso_poisson_loglik(const kcso_config *c, const double *y, const double *r, int r_mode,
                            double scale, const double *x);

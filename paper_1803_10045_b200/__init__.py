@@ -32,7 +32,7 @@ PROFILE_CLASSES = ("pack", "unpack", "kinetic", "forward", "back", "lm", "other"
 # every symbol include/kcs.h declares (tests/test_abi.py checks the library exports each of them)
 EXPORTS = ["kcs_create", "kcs_destroy", "kcs_set_stream", "kcs_last_error", "kcs_workspace_bytes", "kcs_get_mask",
            "kcs_launch_count", "kcs_profile_enable", "kcs_profile_read", "kcs_forward_project", "kcs_back_project", "kcs_sensitivity", "kcs_osl_update",
-           "kcs_kinetic_eval", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host"]
+           "kcs_kinetic_eval", "kcs_ki_map", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host"]
 
 
 class KcsError(RuntimeError):
@@ -52,6 +52,7 @@ class _Config(C.Structure):
         ("t_start_min", C.POINTER(C.c_double)), ("t_end_min", C.POINTER(C.c_double)),
         ("feng_A", C.c_float * 3), ("feng_lambda", C.c_float * 3),
         ("mask_host", C.POINTER(C.c_ubyte)),
+        ("n_replicas", C.c_int),
     ]
 
 
@@ -91,6 +92,7 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.kcs_sensitivity.argtypes = [vp, i, fp]
     lib.kcs_osl_update.argtypes = [vp, fp, fp, fp, fp, f, i, f]
     lib.kcs_kinetic_eval.argtypes = [vp, fp, fp, fp]
+    lib.kcs_ki_map.argtypes = [vp, fp, fp]
     lib.kcs_map_lm.argtypes = [vp, fp, fp, fp, f, f, i, fp]
     lib.kcs_icm_iteration.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, i]
     lib.kcs_icm_run.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, f, i, i]
@@ -152,7 +154,9 @@ class Context:
         c.feng_A = (C.c_float * 3)(*cfg["feng_A"])
         c.feng_lambda = (C.c_float * 3)(*cfg["feng_lambda"])
         c.mask_host = None if mask is None else self._keep[2].ctypes.data_as(C.POINTER(C.c_ubyte))
-        self.nx, self.ny, self.nz = c.nx, c.ny, c.nz
+        c.n_replicas = int(cfg.get("n_replicas", 1))
+        self.n_replicas = max(1, c.n_replicas)
+        self.nx, self.ny, self.nz = c.nx, c.ny, c.nz * self.n_replicas  # nz: all slices (replica-major)
         self.A, self.B, self.S, self.T = c.n_angles, c.n_bins, c.n_subsets, c.n_frames
         self.V = self.nx * self.ny * self.nz
         if stream is None:
@@ -235,6 +239,11 @@ class Context:
         self._check(self._lib.kcs_kinetic_eval(self._h, _dev(theta, (4,) + shp), _dev(F, (self.T,) + shp),
                                                None if J is None else _dev(J, (4, self.T) + shp)))
         return F
+
+    def ki_map(self, theta, ki):
+        shp = (self.nz, self.ny, self.nx)
+        self._check(self._lib.kcs_ki_map(self._h, _dev(theta, (4,) + shp), _dev(ki, shp)))
+        return ki
 
     def map_lm(self, x, theta, lam, gamma: float, delta: float, n_steps: int, cost=None):
         shp = (self.nz, self.ny, self.nx)

@@ -72,7 +72,7 @@ void fill_boundary(const Feng &fe, double t, KBoundary &b) {
 
 int check_cfg(const kcs_config *c, std::string &why) {
     if (c->nx <= 0 || c->ny <= 0 || c->nz <= 0 || c->n_angles <= 0 || c->n_bins < 5 || c->n_steps <= 0 ||
-        c->n_subsets <= 0 || !(c->vx > 0) || !(c->vy > 0) || !(c->bin_mm > 0) || !(c->step_mm > 0)) {
+        c->n_subsets <= 0 || c->n_replicas < 0 || !(c->vx > 0) || !(c->vy > 0) || !(c->bin_mm > 0) || !(c->step_mm > 0)) {
         why = "non-positive size (n_bins must be >= 5: the back-projector reads 5-bin windows)";
         return KCS_ERR_SHAPE;
     }
@@ -257,9 +257,10 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->st_y = c->st_r = c->st_x = c->st_theta = c->st_lambda = nullptr;
     c->st_r_elems = 0;
 
-    const int nx = cfg->nx, ny = cfg->ny, nz = cfg->nz, A = cfg->n_angles, B = cfg->n_bins, K = cfg->n_steps, T = cfg->n_frames;
+    const int nrep = cfg->n_replicas > 0 ? cfg->n_replicas : 1;
+    const int nx = cfg->nx, ny = cfg->ny, nz = cfg->nz * nrep, A = cfg->n_angles, B = cfg->n_bins, K = cfg->n_steps, T = cfg->n_frames;
     KGeom &g = c->g;
-    g.nx = nx; g.ny = ny; g.nz = nz; g.nxp = nx + 2 * KCS_PAD; g.nyp = ny + 2 * KCS_PAD;
+    g.nx = nx; g.ny = ny; g.nz = nz; g.nzr = cfg->nz; g.nxp = nx + 2 * KCS_PAD; g.nyp = ny + 2 * KCS_PAD;
     g.A = A; g.B = B; g.K = K; g.S = cfg->n_subsets;
     g.step_mm = cfg->step_mm; g.bin_mm = cfg->bin_mm;
     g.cx = 0.5 * (nx - 1); g.cy = 0.5 * (ny - 1); g.cb = 0.5 * (B - 1); g.ck = 0.5 * (K - 1);
@@ -438,6 +439,12 @@ int kcs_osl_update(kcs_ctx *c, float *x, const float *bp, const float *sens, con
         return fail(c, KCS_ERR_SHAPE, "kcs_osl_update: unknown prior_mode");
     if (prior_mode == KCS_PRIOR_ABSOLUTE && !(sigma2 > 0.f)) return fail(c, KCS_ERR_SHAPE, "kcs_osl_update: sigma2 <= 0");
     return kcs_launch_osl_planar(c, x, bp, sens, F, beta, prior_mode, sigma2);
+}
+
+int kcs_ki_map(kcs_ctx *c, const float *theta, float *ki) {
+    if (!c) return KCS_ERR_NULL;
+    if (!theta || !ki) return fail(c, KCS_ERR_NULL, "kcs_ki_map: NULL buffer");
+    return kcs_launch_ki_map(c, theta, ki);
 }
 
 int kcs_kinetic_eval(kcs_ctx *c, const float *theta, float *F, float *J) {

@@ -18,7 +18,8 @@
 #define KCS_PAD 2  // zero pixels around every slice of the padded layout
 
 struct KGeom {
-    int nx, ny, nz;
+    int nx, ny, nz;    // nz = ALL slices (replicas x slices per replica)
+    int nzr;           // slices per replica: z-neighbours exist only inside [k nzr, (k+1) nzr)
     int nxp, nyp;      // nx + 2 KCS_PAD, ny + 2 KCS_PAD
     int A, B, K, S;
     float step_mm, bin_mm;
@@ -179,6 +180,7 @@ int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *se
 // ---- launchers (kcs_kinetic.cu) ------------------------------------------------------------------
 // F (and J) from theta.  inner == 0: F planar [T][V], J planar [4][T][V] or NULL;  inner == 1: F = padded inner layout, Tp.
 int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp);
+int kcs_launch_ki_map(kcs_ctx *c, const float *theta, float *ki);
 // one Jacobi LM step: reads theta_in, writes theta_out for the in-mask voxels (masked-out voxels are never touched).
 //   x_inner == 0: x planar [T][V];  x_inner == 1: x = c->xi padded inner layout with Tp.
 int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const void *theta_in, int in_f64, void *theta_out,

@@ -306,7 +306,8 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
 #pragma unroll
         for (int q = 0; q < 6; ++q) {
             const int ii = i + di[q], jj = j + dj[q], zz = z + dz[q];
-            const bool ok = ii >= 0 && ii < g.nx && jj >= 0 && jj < g.ny && zz >= 0 && zz < g.nz && mask[jj * g.nx + ii];
+            const bool ok = ii >= 0 && ii < g.nx && jj >= 0 && jj < g.ny && zz >= 0 && zz < g.nz && zz / g.nzr == z / g.nzr &&
+                            mask[jj * g.nx + ii];  // in-volume, in the same replica, in-mask
             if (ok) {
                 const size_t w = (size_t)zz * v2 + (size_t)jj * g.nx + ii;
 #pragma unroll
@@ -376,7 +377,24 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
     if (cost) cost[v] = (float)phi;
 }
 
+// K_i = K1 k3 / (k2 + k3)
+__global__ void k_ki_map(const float *__restrict__ theta, float *__restrict__ ki, long long nvox) {
+    const long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= nvox) return;
+    const float K1 = theta[v], k2 = theta[nvox + v], k3 = theta[2 * nvox + v];
+    const float a = k2 + k3;
+    ki[v] = a > 0.f ? K1 * k3 / a : 0.f;
+}
+
 }  // namespace
+
+int kcs_launch_ki_map(kcs_ctx *c, const float *theta, float *ki) {
+    const long long nvox = (long long)c->n_vox;
+    ProfScope ps(c, KCS_K_OTHER);
+    k_ki_map<<<(unsigned)((nvox + 255) / 256), 256, 0, c->stream>>>(theta, ki, nvox);
+    LAUNCH_CHECK(c);
+    return KCS_OK;
+}
 
 int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp) {
     const long long nvox = (long long)c->n_vox;
