@@ -24,7 +24,8 @@ single-GPU configuration (BASELINE's `metric` names no config).
              ones (rays clipped to the field of view, in-mask voxels); the defined operation's count is printed too.
   cpu_baseline  the fp64 oracle (oracle/, as it stands) on this box's host cores: one ICM iteration of a bounded
              sample (a few slices) of the same workload.
-  per_config ICM it/s of the other configurations (C1, C2, C3), unless --no-per-config.
+  per_config ICM it/s of the other configurations (C1, C2, C3) and of C1 as one batch of 100 noise realisations
+             (kcs_config.n_replicas), unless --no-per-config.
   sweeps     C5(a)/(b) kernel sweeps on the C4 geometry (projector Gsamples/s by frames per launch, MAP-LM fits/s by
              gamma), each with its roofline fraction, unless --no-sweeps.
 
@@ -335,6 +336,32 @@ def time_config(torch, kcs, dev, name: str, steps: int, warmup: int) -> dict:
     return out
 
 
+def time_replicas(torch, kcs, dev, name: str, n_rep: int, steps: int, warmup: int) -> dict:
+    """`n_rep` Poisson realisations of one small workload reconstructed in ONE batch
+    (kcs_config.n_replicas): every launch covers n_rep x nz slices, so the launch-bound small configurations fill the GPU.
+    Reports ICM iterations/s of the batch and replica-iterations/s."""
+    base = ki.config(name)
+    one = kcs.Context(base)
+    _, prob, (x0, th0, lam0) = build_problem(one, base, torch, noisy=False)
+    one.close()
+    cfg = dict(base, n_replicas=n_rep)
+    ctx = kcs.Context(cfg)
+    batch = dict(prob, y=ki.noise_realisations(prob["ybar"], base["seed"], n_rep))
+    st = (ki.tile_replicas(x0, 1, n_rep), ki.tile_replicas(th0, 1, n_rep), ki.tile_replicas(lam0, 0, n_rep))
+    run = IcmRunner(torch, ctx, dict(cfg, nz=base["nz"] * n_rep), batch, st, dev)
+    run.run(warmup)
+    torch.cuda.synchronize()
+    n0 = ctx.launch_count()
+    evs = run.run(steps)
+    torch.cuda.synchronize()
+    ms = float(sum(a.elapsed_time(b) for a, b in evs))
+    out = {"replicas": n_rep, "it_s": steps / ms * 1e3, "replica_it_s": n_rep * steps / ms * 1e3, "ms_per_iteration": ms / steps,
+           "steps": steps, "warmup": warmup, "gpu_launches_per_iteration": (ctx.launch_count() - n0) / steps, "l2": run.l2_note,
+           "finite": bool(torch.isfinite(run.x).all() and torch.isfinite(run.th).all())}
+    ctx.close()
+    return out
+
+
 # ------------------------------------------------------------------------------------------------ our arm
 def run_ours(args):
     import torch
@@ -454,6 +481,10 @@ def run_ours(args):
                     result["per_config"][name] = time_config(torch, kcs, dev, name, 10 if name != "C4" else 10, 3)
                 except Exception as e:
                     result["per_config"][name] = {"error": repr(e)}
+            try:  # the launch-bound C1 (S:7-H6) as a batch of 100 noise realisations
+                result["per_config"]["C1 x 100 replicas"] = time_replicas(torch, kcs, dev, "C1", 100, 10, 3)
+            except Exception as e:
+                result["per_config"]["C1 x 100 replicas"] = {"error": repr(e)}
         if not args.no_sweeps:
             try:
                 result["sweeps"] = run_sweeps(torch, kcs, dev, peaks)
