@@ -228,19 +228,31 @@ class Oracle:
         assert r.size == self.T * self.nz * self.A * self.B
         return r, 1
 
-    def os_pass(self, y, r, scale, x, F, beta):
+    def os_pass(self, y, r, scale, x, F, beta, mult=None):
+        """mult: multiplicative sinogram [nz][A][B] (attenuation x normalisation, S8(f)3), None = unity."""
         y, x, F = _f64(y), _f64(x).copy(), _f64(F)
         r, mode = self._r(r)
-        _L().kcso_os_pass(self.ref, _p(y), _p(r), C.c_int(mode), C.c_double(scale), _p(x), _p(F),
-                          C.c_double(beta))
+        if mult is None:
+            _L().kcso_os_pass(self.ref, _p(y), _p(r), C.c_int(mode), C.c_double(scale), _p(x), _p(F), C.c_double(beta))
+        else:
+            mult = _f64(mult)
+            assert mult.size == self.nz * self.A * self.B
+            _L().kcso_os_pass_mult(self.ref, _p(y), _p(r), C.c_int(mode), C.c_double(scale), _p(mult), _p(x), _p(F),
+                                   C.c_double(beta))
         return x.reshape(self.T, self.nz, self.ny, self.nx)
 
-    def icm_iteration(self, y, r, scale, x, theta, lam, beta, gamma, delta, n_lm):
+    def icm_iteration(self, y, r, scale, x, theta, lam, beta, gamma, delta, n_lm, mult=None):
         y, x = _f64(y), _f64(x).copy()
         theta, lam = _f64(theta).copy(), _f64(lam).copy()
         r, mode = self._r(r)
-        _L().kcso_icm_iteration(self.ref, _p(y), _p(r), C.c_int(mode), C.c_double(scale), _p(x), _p(theta),
-                                _p(lam), C.c_double(beta), C.c_double(gamma), C.c_double(delta), C.c_int(n_lm))
+        if mult is None:
+            _L().kcso_icm_iteration(self.ref, _p(y), _p(r), C.c_int(mode), C.c_double(scale), _p(x), _p(theta),
+                                    _p(lam), C.c_double(beta), C.c_double(gamma), C.c_double(delta), C.c_int(n_lm))
+        else:
+            mult = _f64(mult)
+            assert mult.size == self.nz * self.A * self.B
+            _L().kcso_icm_iteration_mult(self.ref, _p(y), _p(r), C.c_int(mode), C.c_double(scale), _p(mult), _p(x), _p(theta),
+                                         _p(lam), C.c_double(beta), C.c_double(gamma), C.c_double(delta), C.c_int(n_lm))
         return (x.reshape(self.T, self.nz, self.ny, self.nx),
                 theta.reshape(4, self.nz, self.ny, self.nx), lam.reshape(self.nz, self.ny, self.nx))
 

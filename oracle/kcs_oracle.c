@@ -658,6 +658,77 @@ void kcso_os_pass(const kcso_config *c, const double *y, const double *r, int r_
     free(sens);
 }
 
+/* ------------------------------------------------------------------------------------------
+ * S8(f)3 -- P:49 "all effects of attenuation, scatter and randoms": a frame-independent multiplicative sinogram
+ * n[nz][A][B] (attenuation x normalisation factors) enters the acquisition model,
+ *   yhat = scale n (A_s x_t) + r_t ;  q = y/yhat where yhat > 1e-12 else 0 ;  b = scale A_s^T (n q) ;  S_s = scale A_s^T n.
+ * Scatter is additive and enters through r (r_mode 1).  The sensitivity now differs from slice to slice; O2 is otherwise
+ * unchanged, with max(S_s) taken over the whole volume.  mult == NULL is kcso_os_pass.
+ * ------------------------------------------------------------------------------------------ */
+void kcso_os_pass_mult(const kcso_config *c, const double *y, const double *r, int r_mode, double scale, const double *mult,
+                       double *x, const double *F, double beta) {
+    if (!mult) { kcso_os_pass(c, y, r, r_mode, scale, x, F, beta); return; }
+    const int T = c->n_frames, S = c->n_subsets, A = c->n_angles, B = c->n_bins, As = A / S;
+    const size_t V2 = (size_t)c->nx * c->ny, V = V2 * c->nz;
+    const size_t Rs = (size_t)c->nz * As * B; /* rays per frame in one subset */
+    double *yh = (double *)malloc(sizeof(double) * T * Rs);
+    double *bp = (double *)malloc(sizeof(double) * T * V);
+    double *sens = (double *)malloc(sizeof(double) * V);
+    double *ns = (double *)malloc(sizeof(double) * Rs);
+    unsigned char *owned;
+    const unsigned char *mask = get_mask(c, &owned);
+    for (int s = 0; s < S; ++s) {
+        for (int z = 0; z < c->nz; ++z)          /* n restricted to the subset's angles */
+            for (int la = 0; la < As; ++la)
+                for (int b = 0; b < B; ++b)
+                    ns[((size_t)z * As + la) * B + b] = mult[((size_t)z * A + (s + la * S)) * B + b];
+        kcso_forward_project(c, x, yh, s, T);
+        for (int t = 0; t < T; ++t)
+            for (int z = 0; z < c->nz; ++z)
+                for (int la = 0; la < As; ++la)
+                    for (int b = 0; b < B; ++b) {
+                        const size_t is = (((size_t)t * c->nz + z) * As + la) * B + b;
+                        const int a = s + la * S;
+                        const size_t ifull = (((size_t)t * c->nz + z) * A + a) * B + b;
+                        const double n = ns[((size_t)z * As + la) * B + b];
+                        const double rr = r_mode == 0 ? r[t] : r[ifull];
+                        const double yhat = scale * n * yh[is] + rr;
+                        yh[is] = yhat > 1e-12 ? n * y[ifull] / yhat : 0.0;   /* n q: what the transpose acts on */
+                    }
+        kcso_back_project(c, yh, bp, s, T);
+        for (size_t q = 0; q < (size_t)T * V; ++q) bp[q] *= scale;
+        for (int z = 0; z < c->nz; ++z) back_project_slice(c, ns + (size_t)z * As * B, sens + (size_t)z * V2, s);
+        double smax = 0.0;
+        for (size_t p = 0; p < V; ++p) { sens[p] *= scale; if (sens[p] > smax) smax = sens[p]; }
+        for (int t = 0; t < T; ++t)
+            for (size_t v = 0; v < V; ++v) {
+                const size_t idx = (size_t)t * V + v;
+                const double Sv = sens[v];
+                if (!mask[v % V2] || Sv <= 1e-12 * smax) { x[idx] = 0.0; continue; }
+                double D = Sv * (1.0 + beta * (x[idx] - F[idx]) / fmax(F[idx], 1e-20));
+                D = fmax(D, 0.1 * Sv);
+                x[idx] = x[idx] * bp[idx] / D;
+            }
+    }
+    free(owned);
+    free(yh);
+    free(bp);
+    free(sens);
+    free(ns);
+}
+
+void kcso_icm_iteration_mult(const kcso_config *c, const double *y, const double *r, int r_mode, double scale,
+                             const double *mult, double *x, double *theta, double *lambda,
+                             double beta, double gamma, double delta, int n_lm) {
+    const int T = c->n_frames;
+    const size_t V = (size_t)c->nx * c->ny * c->nz;
+    double *F = (double *)malloc(sizeof(double) * T * V);
+    kcso_kinetic_eval(c, theta, F, NULL, (long)V);
+    kcso_os_pass_mult(c, y, r, r_mode, scale, mult, x, F, beta);
+    kcso_map_lm(c, x, theta, lambda, gamma, delta, n_lm, NULL);
+    free(F);
+}
+
 void kcso_icm_iteration(const kcso_config *c, const double *y, const double *r, int r_mode, double scale,
                         double *x, double *theta, double *lambda,
                         double beta, double gamma, double delta, int n_lm) {

@@ -94,6 +94,14 @@ void kcso_os_pass(const kcso_config *c, const double *y, const double *r, int r_
 void kcso_icm_iteration(const kcso_config *c, const double *y, const double *r, int r_mode, double scale,
                         double *x, double *theta, double *lambda,
                         double beta, double gamma, double delta, int n_lm);
+/* S8(f)3: the same with a multiplicative sinogram mult[nz][A][B] (attenuation x normalisation; NULL = unity):
+ * yhat = scale mult (A_s x) + r, b = scale A_s^T (mult q), S_s = scale A_s^T mult (per slice). */
+void kcso_os_pass_mult(const kcso_config *c, const double *y, const double *r, int r_mode, double scale, const double *mult,
+                       double *x, const double *F, double beta);
+void kcso_icm_iteration_mult(const kcso_config *c, const double *y, const double *r, int r_mode, double scale,
+                             const double *mult, double *x, double *theta, double *lambda,
+                             double beta, double gamma, double delta, int n_lm);
+
 /* K_i = K1 k3 / (k2 + k3) for V voxels, theta[4][V]; 0 where k2 + k3 = 0. */
 void kcso_ki_map(const double *theta, double *ki, long V);
 
