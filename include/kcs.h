@@ -138,6 +138,14 @@ int kcs_map_lm(kcs_ctx *ctx, const float *x, float *theta, float *lambda, float 
  * theta[4][nz][ny][nx]; ki[nz][ny][nx] (device).  Evaluated for every voxel. */
 int kcs_ki_map(kcs_ctx *ctx, const float *theta, float *ki);
 
+/* P:49 "all effects of attenuation, scatter and randoms".  A frame-independent multiplicative sinogram
+ * mult[nz][A][B] (device; attenuation x normalisation factors of every line of response) for the kcs_icm_* calls that
+ * follow:   yhat = scale mult (A_s x) + r,   b = scale A_s^T (mult q),   S_s = scale A_s^T mult  (per slice).
+ * The library keeps its own copy and builds the S per-slice sensitivity volumes (n_subsets * nz*ny*nx floats of
+ * workspace).  NULL restores unit factors.  Scatter is additive: pass randoms + scatter as r with KCS_R_FULL.
+ * kcs_forward_project / kcs_back_project / kcs_sensitivity stay the bare operators A, A^T. */
+int kcs_set_multiplicative(kcs_ctx *ctx, const float *mult);
+
 /* I: one ICM iteration,
  *   F <- K(theta);  for s = 0..S-1: yhat = scale A_s x + r, q = y/yhat (0 where yhat <= 1e-12),
  *   x <- OSL(x, scale A_s^T q, scale A_s^T 1, F, beta);  theta <- n_lm MAP-LM steps on the new x.

@@ -184,6 +184,19 @@ def tile_replicas(a: np.ndarray, axis: int, n: int) -> np.ndarray:
     return np.concatenate([a] * n, axis=axis)
 
 
+MU_WATER_511KEV = 0.0096  # 1/mm, linear attenuation coefficient of water / soft tissue at 511 keV
+
+
+def attenuation_factors(cfg: dict, forward_project) -> np.ndarray:
+    """SURVEY 8(f)3 stand-in for a measured attenuation map: the head of the phantom (every labelled tissue) is
+    water, n[z,a,b] = exp(-mu * chord length) with the chord lengths from the caller's forward projector applied to the
+    head's indicator image (mm).  Returns [nz, A, B] in (0, 1]."""
+    lab, _ = phantom(cfg)
+    head = (lab > 0).astype(np.float64)
+    chord = np.asarray(forward_project(head[None]), dtype=np.float64)[0]
+    return np.exp(-MU_WATER_511KEV * chord)
+
+
 def lm_start(theta_true: np.ndarray, seed: int) -> np.ndarray:
     """C5(b): initial parameters uniform within +/-50 % of the truth."""
     rng = np.random.Generator(np.random.PCG64(seed))

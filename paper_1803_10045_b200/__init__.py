@@ -32,7 +32,7 @@ PROFILE_CLASSES = ("pack", "unpack", "kinetic", "forward", "back", "lm", "other"
 # every symbol include/kcs.h declares (tests/test_abi.py checks the library exports each of them)
 EXPORTS = ["kcs_create", "kcs_destroy", "kcs_set_stream", "kcs_last_error", "kcs_workspace_bytes", "kcs_get_mask",
            "kcs_launch_count", "kcs_profile_enable", "kcs_profile_read", "kcs_forward_project", "kcs_back_project", "kcs_sensitivity", "kcs_osl_update",
-           "kcs_kinetic_eval", "kcs_ki_map", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host"]
+           "kcs_kinetic_eval", "kcs_ki_map", "kcs_set_multiplicative", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host"]
 
 
 class KcsError(RuntimeError):
@@ -93,6 +93,7 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.kcs_osl_update.argtypes = [vp, fp, fp, fp, fp, f, i, f]
     lib.kcs_kinetic_eval.argtypes = [vp, fp, fp, fp]
     lib.kcs_ki_map.argtypes = [vp, fp, fp]
+    lib.kcs_set_multiplicative.argtypes = [vp, fp]
     lib.kcs_map_lm.argtypes = [vp, fp, fp, fp, f, f, i, fp]
     lib.kcs_icm_iteration.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, i]
     lib.kcs_icm_run.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, f, i, i]
@@ -239,6 +240,10 @@ class Context:
         self._check(self._lib.kcs_kinetic_eval(self._h, _dev(theta, (4,) + shp), _dev(F, (self.T,) + shp),
                                                None if J is None else _dev(J, (4, self.T) + shp)))
         return F
+
+    def set_multiplicative(self, mult):
+        """mult: float32 CUDA tensor [nz][A][B] (attenuation x normalisation factors) or None for unit factors."""
+        self._check(self._lib.kcs_set_multiplicative(self._h, None if mult is None else _dev(mult, (self.nz, self.A, self.B))))
 
     def ki_map(self, theta, ki):
         shp = (self.nz, self.ny, self.nx)

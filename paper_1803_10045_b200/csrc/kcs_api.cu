@@ -207,7 +207,7 @@ int kcs_get_mask(const kcs_ctx *ctx, unsigned char *out) {
 int kcs_destroy(kcs_ctx *c) {
     if (!c) return KCS_ERR_NULL;
     cudaStreamSynchronize(c->stream);
-    void *ptrs[] = {c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->d_wtab, c->d_vlist, c->xi, c->Fi,
+    void *ptrs[] = {c->d_mult, c->d_sens_z, c->d_smax_z, c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->d_wtab, c->d_vlist, c->xi, c->Fi,
                     c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->thD[0], c->thD[1], c->lamD, c->lm_state, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
     for (void *p : ptrs)
         if (p) cudaFree(p);
@@ -247,6 +247,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->xi_border_tp = 0;
     c->d_fwd = c->d_bwd = nullptr; c->d_frames = nullptr; c->d_mask = nullptr;
     c->d_sens = c->d_smax = c->d_tmp_smax = nullptr;
+    c->d_mult = c->d_sens_z = c->d_smax_z = nullptr;
     c->d_wtab = nullptr;
     c->d_vlist = nullptr; c->n_inmask2 = 0;
     c->xi = c->Fi = c->qi = c->yi = c->ri = c->r_pad = c->theta2 = nullptr;
@@ -428,6 +429,41 @@ int kcs_sensitivity(kcs_ctx *c, int subset, float *sens) {
     const size_t v2 = (size_t)c->g.nx * c->g.ny;
     const int sidx = subset < 0 ? c->g.S : subset;
     KCS_CUDA_OK(c, cudaMemcpyAsync(sens, c->d_sens + sidx * v2, v2 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    return KCS_OK;
+}
+
+// S8(f)3: the sensitivity images A_s^T n are one plain back-projection of n (as a one-frame sinogram) per subset.
+int kcs_set_multiplicative(kcs_ctx *c, const float *mult) {
+    if (!c) return KCS_ERR_NULL;
+    const KGeom &g = c->g;
+    if (!mult) {  // back to unit factors
+        if (c->d_mult) { cudaStreamSynchronize(c->stream); cudaFree(c->d_mult); c->d_mult = nullptr; }
+        return KCS_OK;
+    }
+    const size_t nr = c->n_ray_all, nv = c->n_vox;
+    cudaError_t e = cudaSuccess;
+    if (!c->d_mult) {
+        e = dalloc(c, &c->d_mult, nr);
+        if (e == cudaSuccess && !c->d_sens_z) e = dalloc(c, &c->d_sens_z, (size_t)g.S * nv);
+        if (e == cudaSuccess && !c->d_smax_z) e = dalloc(c, &c->d_smax_z, (size_t)g.S);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            if (c->d_mult) { cudaFree(c->d_mult); c->d_mult = nullptr; }
+            return fail(c, KCS_ERR_ALLOC, "kcs_set_multiplicative: cannot allocate the per-slice sensitivity images");
+        }
+    }
+    KCS_CUDA_OK(c, cudaMemcpyAsync(c->d_mult, mult, nr * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    const int Tp = 4, As = g.A / g.S;
+    int rc;
+    if ((rc = ensure_border(c, Tp))) return rc;
+    float *rows = c->yi;  // scratch: the packed-data buffer is rewritten by the next kcs_icm_* call anyway
+    for (int s = 0; s < g.S; ++s) {
+        if ((rc = kcs_launch_subset_rows(c, c->d_mult, rows, s))) return rc;
+        if ((rc = pack_sino(c, rows, 1, c->qi, Tp, As))) return rc;
+        if ((rc = kcs_launch_back(c, Tp, s, 0, c->xi, 1.f, 0.f, 0, g.nz))) return rc;
+        if ((rc = unpack_image(c, c->xi, Tp, c->d_sens_z + (size_t)s * nv, 1))) return rc;
+        if ((rc = kcs_launch_max_nonneg(c, c->d_sens_z + (size_t)s * nv, nv, c->d_smax_z + s))) return rc;
+    }
     return KCS_OK;
 }
 

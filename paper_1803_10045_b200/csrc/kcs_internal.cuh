@@ -85,6 +85,8 @@ struct kcs_ctx {
     float *d_sens;                    // [S+1][ny][nx], unscaled A_s^T 1; entry S = all angles
     float *d_smax;                    // [S+1] max over the image of d_sens[s]
     float *d_tmp_smax;                // [1] scratch for kcs_osl_update
+    // S8(f)3 (kcs_set_multiplicative): n[nz][A][B], unscaled A_s^T n per subset and slice [S][nz][ny][nx], their maxima [S]
+    float *d_mult, *d_sens_z, *d_smax_z;
     float4 *d_wtab;                   // back-projector weight table [A][nbj][nbi4][6][4] (k_build_wtab)
     int nbi, nbj, nbi4;               // 2x2 voxel blocks in x, y; groups of 4 blocks in x
 
@@ -173,6 +175,8 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
 //   osl == 1:  c->xi <- OSL update with bp = scale*step*sum, sens = scale*A_s^T 1, F = c->Fi   (O2)
 int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, float scale, float beta, int z0, int nzc);
 int kcs_launch_sens(kcs_ctx *c);  // fills d_sens, d_smax
+int kcs_launch_subset_rows(kcs_ctx *c, const float *n, float *out, int s);  // out[z][la][b] = n[z][s + la S][b]
+int kcs_launch_max_nonneg(kcs_ctx *c, const float *v, size_t n, float *out);  // *out = max(0, max v)
 int kcs_launch_build_wtab(kcs_ctx *c);  // fills d_wtab
 int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *sens, const float *F, float beta,
                           int prior_mode, float sigma2);

@@ -112,6 +112,7 @@ struct FwdArgs {
     const float *yi;     // packed measured sinogram [nz][A][B][Tp]       (ratio only)
     const float *ri;     // packed randoms, same layout                    (ratio, KCS_R_FULL)
     const float *r_pad;  // [32] per-frame randoms, 0 beyond T             (ratio, KCS_R_PER_FRAME)
+    const float *mult;   // [nz][A][B] multiplicative sinogram (attenuation x normalisation) or NULL  (ratio only)
     int Tp, FG, BINS, KSPLIT, KCH, FB;
     int As, subset;
     int ratio, r_mode;
@@ -233,7 +234,9 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, 1) k_forward(KGeom g, FwdArgs p) 
     } else {
         // O1: yhat = scale A_s x + r ; q = y / yhat where yhat > 1e-12 else 0
         const size_t oy = (((size_t)z * g.A + a) * g.B + b) * Tp + fg * FPT;
-        const float sc = p.scale * g.step_mm;
+        // S8(f)3: yhat = scale n (A x) + r and the transpose acts on n q (n = attenuation x normalisation of this ray)
+        const float nm = p.mult ? __ldg(p.mult + ((size_t)z * g.A + a) * g.B + b) : 1.f;
+        const float sc = p.scale * g.step_mm * nm;
 #pragma unroll
         for (int q = 0; q < FPT / 4; ++q) {
             const float4 yv = __ldg(reinterpret_cast<const float4 *>(p.yi + oy) + q);
@@ -244,10 +247,10 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, 1) k_forward(KGeom g, FwdArgs p) 
                 rv = __ldg(reinterpret_cast<const float4 *>(p.ri + oy) + q);
             float4 out;
             float yh;
-            yh = fmaf(sc, acc[4 * q + 0], rv.x); out.x = yh > 1e-12f ? yv.x / yh : 0.f;
-            yh = fmaf(sc, acc[4 * q + 1], rv.y); out.y = yh > 1e-12f ? yv.y / yh : 0.f;
-            yh = fmaf(sc, acc[4 * q + 2], rv.z); out.z = yh > 1e-12f ? yv.z / yh : 0.f;
-            yh = fmaf(sc, acc[4 * q + 3], rv.w); out.w = yh > 1e-12f ? yv.w / yh : 0.f;
+            yh = fmaf(sc, acc[4 * q + 0], rv.x); out.x = yh > 1e-12f ? nm * yv.x / yh : 0.f;
+            yh = fmaf(sc, acc[4 * q + 1], rv.y); out.y = yh > 1e-12f ? nm * yv.y / yh : 0.f;
+            yh = fmaf(sc, acc[4 * q + 2], rv.z); out.z = yh > 1e-12f ? nm * yv.z / yh : 0.f;
+            yh = fmaf(sc, acc[4 * q + 3], rv.w); out.w = yh > 1e-12f ? nm * yv.w / yh : 0.f;
             reinterpret_cast<float4 *>(p.qi + o)[q] = out;
         }
     }
@@ -267,6 +270,7 @@ int kcs_launch_forward(kcs_ctx *c, int Tp, int subset, int ratio, float scale, i
     p.yi = c->yi + (size_t)z0 * g.A * g.B * Tp;
     p.ri = c->ri ? c->ri + (size_t)z0 * g.A * g.B * Tp : nullptr;
     p.r_pad = c->r_pad;
+    p.mult = (ratio && c->d_mult) ? c->d_mult + (size_t)z0 * g.A * g.B : nullptr;
     p.subset = subset;
     p.ratio = ratio; p.r_mode = r_mode; p.scale = scale;
     p.clip_r2 = clip_fov ? c->fov_rc2 : -1.f;
@@ -365,7 +369,8 @@ struct BackArgs {
     const float *qi;
     float *out;          // padded inner layout (plain back-projection) or xi (OSL, in place)
     const float *Fi;
-    const float *sens;   // [ny][nx] unscaled A_s^T 1 of this subset
+    const float *sens;   // [ny][nx] unscaled A_s^T 1 of this subset, or [nz][ny][nx] unscaled A_s^T n (sens_z = 1)
+    int sens_z;
     const float *smax;   // device scalar: max(sens)
     const unsigned char *mask;
     const float4 *wtab;  // [A][nbj][nbi4][KCS_BW][4] block-angle weight records (k_build_wtab)
@@ -539,22 +544,23 @@ __global__ void __launch_bounds__(KCS_BACK_TPB, 4) k_back(KGeom g, BackArgs p) {
     // thread are requested first (they come from L2 / HBM), then updated and stored: one wait instead of 4 ZB.
     const float smax = *p.smax;
     const float sc = p.scale * g.step_mm;
+    const size_t v2 = (size_t)g.nx * g.ny;
     float4 xv[4][ZB], Fv[4][ZB];
-    float Sv[4];
-    bool live[4];
+    float Sv[4][ZB];
+    bool live[4][ZB];
 #pragma unroll
     for (int v = 0; v < 4; ++v) {
         const int i = min(i0 + (v & 1), g.nx - 1), j = min(j0 + (v >> 1), g.ny - 1);
-        const float S0 = p.sens[j * g.nx + i];
-        Sv[v] = p.scale * S0;
-        live[v] = vact[v] && (S0 > 1e-12f * smax);
 #pragma unroll
         for (int zb = 0; zb < ZB; ++zb) {
             const int z = min(z0 + zb, g.nz - 1);
+            const float S0 = p.sens[(p.sens_z ? (size_t)z * v2 : 0) + (size_t)j * g.nx + i];
+            Sv[v][zb] = p.scale * S0;
+            live[v][zb] = vact[v] && (S0 > 1e-12f * smax);
             const size_t o = (((size_t)z * g.nyp + (j + KCS_PAD)) * g.nxp + (i + KCS_PAD)) * Tp + fg * 4;
             xv[v][zb] = make_float4(0.f, 0.f, 0.f, 0.f);
             Fv[v][zb] = make_float4(1.f, 1.f, 1.f, 1.f);
-            if (live[v]) {
+            if (live[v][zb]) {
                 xv[v][zb] = *reinterpret_cast<const float4 *>(p.out + o);
                 Fv[v][zb] = __ldg(reinterpret_cast<const float4 *>(p.Fi + o));
             }
@@ -570,11 +576,11 @@ __global__ void __launch_bounds__(KCS_BACK_TPB, 4) k_back(KGeom g, BackArgs p) {
             if (z >= g.nz) break;
             const size_t o = (((size_t)z * g.nyp + (j + KCS_PAD)) * g.nxp + (i + KCS_PAD)) * Tp + fg * 4;
             float4 out = make_float4(0.f, 0.f, 0.f, 0.f);  // outside the mask or without sensitivity: x = 0 (Q2, Q10)
-            if (live[v]) {
-                out.x = osl_one(xv[v][zb].x, sc * acc[zb][v][0], Fv[v][zb].x, Sv[v], p.beta);
-                out.y = osl_one(xv[v][zb].y, sc * acc[zb][v][1], Fv[v][zb].y, Sv[v], p.beta);
-                out.z = osl_one(xv[v][zb].z, sc * acc[zb][v][2], Fv[v][zb].z, Sv[v], p.beta);
-                out.w = osl_one(xv[v][zb].w, sc * acc[zb][v][3], Fv[v][zb].w, Sv[v], p.beta);
+            if (live[v][zb]) {
+                out.x = osl_one(xv[v][zb].x, sc * acc[zb][v][0], Fv[v][zb].x, Sv[v][zb], p.beta);
+                out.y = osl_one(xv[v][zb].y, sc * acc[zb][v][1], Fv[v][zb].y, Sv[v][zb], p.beta);
+                out.z = osl_one(xv[v][zb].z, sc * acc[zb][v][2], Fv[v][zb].z, Sv[v][zb], p.beta);
+                out.w = osl_one(xv[v][zb].w, sc * acc[zb][v][3], Fv[v][zb].w, Sv[v][zb], p.beta);
             }
             *reinterpret_cast<float4 *>(p.out + o) = out;
         }
@@ -591,8 +597,14 @@ int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, f
     p.out = (osl ? c->xi : out_inner) + zpix;
     p.Fi = c->Fi + zpix;
     const int sidx = subset < 0 ? g.S : subset;
-    p.sens = c->d_sens + (size_t)sidx * g.nx * g.ny;
-    p.smax = c->d_smax + sidx;
+    p.sens_z = (osl && c->d_mult && subset >= 0) ? 1 : 0;
+    if (p.sens_z) {  // S8(f)3: A_s^T n differs from slice to slice
+        p.sens = c->d_sens_z + ((size_t)subset * c->g.nz + z0) * g.nx * g.ny;
+        p.smax = c->d_smax_z + subset;
+    } else {
+        p.sens = c->d_sens + (size_t)sidx * g.nx * g.ny;
+        p.smax = c->d_smax + sidx;
+    }
     p.mask = c->d_mask;
     p.Tp = Tp;
     p.FG = Tp / 4;
@@ -651,9 +663,9 @@ int kcs_launch_sens(kcs_ctx *c) {
 // ---------------------------------------------------------------------------------------------------------
 // Stand-alone OSL update on planar buffers (kcs_osl_update).
 // ---------------------------------------------------------------------------------------------------------
-__global__ void k_max_nonneg(const float *v, int n, float *out) {
+__global__ void k_max_nonneg(const float *v, size_t n, float *out) {
     float m = 0.f;
-    for (int q = blockIdx.x * blockDim.x + threadIdx.x; q < n; q += gridDim.x * blockDim.x) m = fmaxf(m, v[q]);
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) m = fmaxf(m, v[q]);
     for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
     if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<int *>(out), __float_as_int(fmaxf(m, 0.f)));
 }
@@ -678,6 +690,33 @@ __global__ void k_osl_planar(float *x, const float *bp, const float *sens, const
     x[q] = xv * bp[q] / D;
 }
 
+// n[nz][A][B] restricted to the angles of one subset: out[z][la][b] = n[z][s + la S][b]  (one frame of a subset sinogram)
+__global__ void k_subset_rows(const float *__restrict__ n, float *__restrict__ out, int nz, int A, int B, int S, int s) {
+    const int As = A / S;
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= (size_t)nz * As * B) return;
+    const int b = (int)(q % B), la = (int)((q / B) % As), z = (int)(q / ((size_t)B * As));
+    out[q] = n[((size_t)z * A + (s + la * S)) * B + b];
+}
+
+int kcs_launch_subset_rows(kcs_ctx *c, const float *n, float *out, int s) {
+    const KGeom &g = c->g;
+    const size_t tot = (size_t)g.nz * (g.A / g.S) * g.B;
+    ProfScope ps(c, KCS_K_OTHER);
+    k_subset_rows<<<(unsigned)((tot + 255) / 256), 256, 0, c->stream>>>(n, out, g.nz, g.A, g.B, g.S, s);
+    LAUNCH_CHECK(c);
+    return KCS_OK;
+}
+
+int kcs_launch_max_nonneg(kcs_ctx *c, const float *v, size_t n, float *out) {
+    cudaError_t e = cudaMemsetAsync(out, 0, sizeof(float), c->stream);
+    if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return KCS_ERR_CUDA; }
+    ProfScope ps(c, KCS_K_OTHER);
+    k_max_nonneg<<<256, 256, 0, c->stream>>>(v, n, out);
+    LAUNCH_CHECK(c);
+    return KCS_OK;
+}
+
 int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *sens, const float *F, float beta,
                           int prior_mode, float sigma2) {
     const KGeom &g = c->g;
@@ -685,7 +724,7 @@ int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *se
     cudaError_t e = cudaMemsetAsync(c->d_tmp_smax, 0, sizeof(float), c->stream);
     if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return KCS_ERR_CUDA; }
     ProfScope ps(c, KCS_K_OTHER);
-    k_max_nonneg<<<64, 256, 0, c->stream>>>(sens, v2, c->d_tmp_smax);
+    k_max_nonneg<<<64, 256, 0, c->stream>>>(sens, (size_t)v2, c->d_tmp_smax);
     LAUNCH_CHECK(c);
     const size_t n = (size_t)c->cfg.n_frames * c->n_vox;
     k_osl_planar<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(x, bp, sens, F, c->d_mask, c->d_tmp_smax, n, v2, beta,
