@@ -274,6 +274,15 @@ class Oracle:
         return np.concatenate(xs, axis=1), np.concatenate(ths, axis=1), np.concatenate(lams, axis=0)
 
     @staticmethod
+    def set_lm_options(frame_w=None, neighbourhood=6, delta4=None):
+        """S8(f)2 / S8(f)4: weighted least squares, the 3x3-clique neighbourhood (10), per-parameter Huber thresholds.
+        Oracle-wide; call with no arguments to restore the defaults."""
+        fw = None if frame_w is None else _f64(frame_w)
+        d4 = None if delta4 is None else _f64(delta4)
+        _L().kcso_set_lm_options(None if fw is None else _p(fw), C.c_int(0 if fw is None else fw.size), C.c_int(neighbourhood),
+                                 None if d4 is None else _p(d4))
+
+    @staticmethod
     def ki_map(theta):
         """K_i = K1 k3 / (k2 + k3)."""
         theta = _f64(theta)

@@ -473,6 +473,25 @@ static double huber_d(double t, double delta) { /* eq. 6 with Q12: clamp(t,-delt
     return t < -delta ? -delta : (t > delta ? delta : t);
 }
 
+/* S8(f)2 / S8(f)4 options of the fit (oracle-wide knobs like the Q15a slack; defaults = the hot path of S8(a)):
+ *   frame weights w_m >= 0: data term 1/2 sum_m w_m (x_m - F_m)^2, J^T W J, J^T W r (weighted least squares);
+ *   neighbourhood 6 (Q13) or 10: the 8 in-plane neighbours of the paper's 3x3 clique (Fig. 1 caption P:47) plus
+ *     +-z, unit weights, in-volume and in-mask only (free boundary, Q13);
+ *   one Huber threshold per parameter map, delta_p (P:114 applies the potential to each map; the maps differ in scale). */
+#define KCSO_MAX_FRAMES 64
+static double lm_w[KCSO_MAX_FRAMES];
+static int lm_has_w = 0, lm_nbr = 6, lm_has_delta4 = 0;
+static double lm_delta4[4];
+void kcso_set_lm_options(const double *frame_w, int n_frames, int neighbourhood, const double *delta4) {
+    lm_has_w = frame_w != NULL;
+    for (int m = 0; m < KCSO_MAX_FRAMES; ++m) lm_w[m] = (frame_w && m < n_frames) ? frame_w[m] : 1.0;
+    lm_nbr = neighbourhood == 10 ? 10 : 6;
+    lm_has_delta4 = delta4 != NULL;
+    for (int p = 0; p < 4; ++p) lm_delta4[p] = delta4 ? delta4[p] : 0.0;
+}
+static double frame_w(int m) { return lm_has_w ? lm_w[m] : 1.0; }
+static double delta_of(int p, double delta) { return lm_has_delta4 ? lm_delta4[p] : delta; }
+
 static const double BOX_LO[4] = {0.0, 1e-4, 0.0, 0.0};
 static const double BOX_HI[4] = {2.0, 2.0, 1.0, 1.0};
 
@@ -480,9 +499,9 @@ static double objective(const kcso_config *c, const double *xv, const double xi[
                         const double *nbr, int n_nbr, double gamma, double delta) {
     const int T = c->n_frames;
     double phi = 0.0;
-    for (int m = 0; m < T; ++m) phi += 0.5 * (xv[m] - Fv[m]) * (xv[m] - Fv[m]);
+    for (int m = 0; m < T; ++m) phi += 0.5 * frame_w(m) * (xv[m] - Fv[m]) * (xv[m] - Fv[m]);
     for (int p = 0; p < 4; ++p)
-        for (int q = 0; q < n_nbr; ++q) phi += gamma * huber(xi[p] - nbr[q * 4 + p], delta);
+        for (int q = 0; q < n_nbr; ++q) phi += gamma * huber(xi[p] - nbr[q * 4 + p], delta_of(p, delta));
     return phi;
 }
 
@@ -534,9 +553,9 @@ static double lm_step_voxel(const kcso_config *c, const double *tab, const doubl
     double JtJ[4][4] = {{0}}, g[4] = {0};
     for (int p = 0; p < 4; ++p) {
         for (int q = 0; q < 4; ++q)
-            for (int m = 0; m < T; ++m) JtJ[p][q] += Jv[p * T + m] * Jv[q * T + m];
-        for (int m = 0; m < T; ++m) g[p] += Jv[p * T + m] * (xv[m] - Fv[m]);
-        for (int q = 0; q < n_nbr; ++q) g[p] -= gamma * huber_d(xi[p] - nbr[q * 4 + p], delta);
+            for (int m = 0; m < T; ++m) JtJ[p][q] += frame_w(m) * Jv[p * T + m] * Jv[q * T + m];
+        for (int m = 0; m < T; ++m) g[p] += frame_w(m) * Jv[p * T + m] * (xv[m] - Fv[m]);
+        for (int q = 0; q < n_nbr; ++q) g[p] -= gamma * huber_d(xi[p] - nbr[q * 4 + p], delta_of(p, delta));
     }
     if (!(*lam > 0.0)) { /* Q15: first use */
         double mx = 0.0;
@@ -591,10 +610,12 @@ void kcso_map_lm(const kcso_config *c, const double *x, double *theta, double *l
                     if (cost) cost[v] = 0.0;
                     continue;
                 }
-                double nbr[6 * 4];
+                double nbr[10 * 4];
                 int n_nbr = 0;
-                const int di[6] = {-1, 1, 0, 0, 0, 0}, dj[6] = {0, 0, -1, 1, 0, 0}, dz[6] = {0, 0, 0, 0, -1, 1};
-                for (int q = 0; q < 6; ++q) {
+                /* Q13: +-x, +-y, +-z;  neighbourhood 10: the four in-plane diagonals of the 3x3 clique as well */
+                const int di[10] = {-1, 1, 0, 0, 0, 0, -1, 1, -1, 1}, dj[10] = {0, 0, -1, 1, 0, 0, -1, -1, 1, 1},
+                          dz[10] = {0, 0, 0, 0, -1, 1, 0, 0, 0, 0};
+                for (int q = 0; q < lm_nbr; ++q) {
                     const int ii = i + di[q], jj = j + dj[q], zz = z + dz[q];
                     if (ii < 0 || ii >= nx || jj < 0 || jj >= ny || zz < 0 || zz >= nz) continue;
                     if (!mask[(size_t)jj * nx + ii]) continue;

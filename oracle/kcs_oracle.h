@@ -82,6 +82,11 @@ double kcso_lm_objective(const kcso_config *c, const double *xv, const double xi
 void kcso_map_lm(const kcso_config *c, const double *x, double *theta, double *lambda,
                  double gamma, double delta, int n_steps, double *cost);
 
+/* S8(f)2 / S8(f)4 options of the fit, oracle-wide (NULL / 6 / NULL restore the hot path of S8(a)):
+ * frame_w[n_frames] weights of the data term (weighted least squares); neighbourhood 6 (Q13) or 10 (3x3 in-plane clique
+ * of P:114 plus +-z); delta4[4] one Huber threshold per parameter map (the scalar delta argument is then ignored). */
+void kcso_set_lm_options(const double *frame_w, int n_frames, int neighbourhood, const double *delta4);
+
 /* Q15a knob (oracle only): relative slack of the LM acceptance test, default 1e-6. */
 void kcso_set_lm_accept_slack(double s);
 double kcso_get_lm_accept_slack(void);
