@@ -134,6 +134,16 @@ int kcs_kinetic_eval(kcs_ctx *ctx, const float *theta, float *F, float *J);
 int kcs_map_lm(kcs_ctx *ctx, const float *x, float *theta, float *lambda, float gamma, float delta,
                int n_steps, float *cost);
 
+/* Options of the fit beyond the hot path, for the kcs_map_lm / kcs_icm_* calls that follow; all
+ * pointers [host]; SYNCHRONISES the stream.  NULL / 6 / NULL restore the defaults.
+ *   frame_weights[T] >= 0   weighted least squares: data term 1/2 sum_m w_m (x_m - F_m)^2 (e.g. frame-duration or
+ *                           inverse-variance weights); w_m = 0 drops frame m from the fit
+ *   neighbourhood           6: +-x, +-y, +-z (Q13).  10: the 8 in-plane neighbours of the paper's 3x3 clique (P:114,
+ *                           Fig. 1 caption P:47) plus +-z; unit weights, in-volume and in-mask neighbours only
+ *   delta4[4]               one Huber threshold per parameter map (K1, k2, k3, vB); the scalar delta argument of the
+ *                           calls is then ignored */
+int kcs_set_fit_options(kcs_ctx *ctx, const double *frame_weights, int neighbourhood, const double *delta4);
+
 /* the macro-parameter map K_i = K1 k3 / (k2 + k3) (net influx rate; 0 where k2 + k3 = 0) from
  * theta[4][nz][ny][nx]; ki[nz][ny][nx] (device).  Evaluated for every voxel. */
 int kcs_ki_map(kcs_ctx *ctx, const float *theta, float *ki);

@@ -324,6 +324,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
         f.W0 = (double)((long double)f.dt * ICp_ts +
                         gl8([&](long double u) { return ((long double)te - u) * fe.Cp(u); }, ts, te, np));
         f.contiguous = (m > 0 && c->ts[m] == c->te[m - 1]) ? 1 : 0;
+        f.w = 1.0;
         if (m > 0 && std::fabs(f.dt - frames[m - 1].dt) <= 1e-12 * f.dt) {
             f.dt = frames[m - 1].dt;  // same duration class: per-duration scalars are reused (1e-12 relative)
             f.new_dt = 0;
@@ -338,6 +339,10 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
         kin.lam[i] = (double)fe.lam[i];
     }
     kin.beta0 = (double)fe.be[0];
+    c->h_frames = frames;
+    c->nbr_mode = 6;
+    c->has_delta4 = false;
+    c->weighted = false;
 
     std::vector<int> vlist;
     for (int q = 0; q < nx * ny; ++q)
@@ -512,6 +517,27 @@ static int lm_steps(kcs_ctx *c, const float *x, int x_inner, int Tp, float *thet
                                     last ? cost : nullptr);
         if (rc) return rc;
     }
+    return KCS_OK;
+}
+
+int kcs_set_fit_options(kcs_ctx *c, const double *frame_weights, int neighbourhood, const double *delta4) {
+    if (!c) return KCS_ERR_NULL;
+    if (neighbourhood != 6 && neighbourhood != 10) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: neighbourhood must be 6 or 10");
+    const int T = c->cfg.n_frames;
+    for (int m = 0; m < T; ++m)
+        if (frame_weights && !(frame_weights[m] >= 0.0)) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: negative frame weight");
+    for (int p = 0; p < 4; ++p)
+        if (delta4 && !(delta4[p] >= 0.0)) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: negative delta");
+    c->weighted = false;
+    for (int m = 0; m < T; ++m) {
+        c->h_frames[m].w = frame_weights ? frame_weights[m] : 1.0;
+        if (c->h_frames[m].w != 1.0) c->weighted = true;
+    }
+    KCS_CUDA_OK(c, cudaStreamSynchronize(c->stream));  // kernels in flight still read the old table
+    KCS_CUDA_OK(c, cudaMemcpy(c->d_frames, c->h_frames.data(), sizeof(KFrame) * T, cudaMemcpyHostToDevice));
+    c->nbr_mode = neighbourhood;
+    c->has_delta4 = delta4 != nullptr;
+    for (int p = 0; p < 4; ++p) c->delta4[p] = delta4 ? delta4[p] : 0.0;
     return KCS_OK;
 }
 

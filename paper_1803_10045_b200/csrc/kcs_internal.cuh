@@ -47,6 +47,7 @@ struct KFrame {
     double dt;    // t_end - t_start
     int contiguous;  // t_start == previous frame's t_end (state carried over)
     int new_dt;      // dt differs from the previous frame's (per-duration scalars must be recomputed)
+    double w;        // weight of this frame in the least-squares data term (S8(f)4; 1 by default)
 };
 struct KKin {
     int T;
@@ -78,6 +79,11 @@ struct kcs_ctx {
     KKin kin;
     double4 *d_fwd, *d_bwd;
     KFrame *d_frames;
+    std::vector<KFrame> h_frames;     // host copy (kcs_set_fit_options rewrites the frame weights)
+    int nbr_mode;                     // 6 (Q13) or 10 (3x3 in-plane clique + the two axial neighbours, S8(f)2)
+    bool weighted;                    // some frame weight differs from 1 (S8(f)4)
+    bool has_delta4;                  // one Huber threshold per parameter map instead of the scalar argument
+    double delta4[4];
     unsigned char *d_mask;            // [ny][nx]
     int *d_vlist;                     // in-mask pixel indices j*nx+i of one slice, ascending
     int n_inmask2;                    // their count

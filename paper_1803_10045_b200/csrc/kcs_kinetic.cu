@@ -247,17 +247,21 @@ __device__ __forceinline__ bool chol4(const double m[10], const double g[4], dou
 
 // Data part of the normal equations at theta: out[0..9] = J^T J (packed lower triangle), out[10..13] = J^T r,
 // out[14] = 1/2 sum r^2.  One (not inlined) copy of the model code serves both evaluations of a step.
+template <bool WLS>
 __device__ __forceinline__ void lm_eval(KKin kin, const KFrame *fr, const float *__restrict__ x, size_t xbase, size_t xstride,
                                      double K1, double k2, double k3, double vB, double *out) {
     double JtJ[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, gr[4] = {0, 0, 0, 0}, phi = 0.0;
     tac_stream<true>(kin, fr, K1, k2, k3, vB, [&](int m, double Fm, double j0, double j1, double j2, double j3) {
         const double r = (double)x[xbase + m * xstride] - Fm;
-        phi += 0.5 * r * r;
-        JtJ[0] += j0 * j0;
-        JtJ[1] += j1 * j0; JtJ[2] += j1 * j1;
-        JtJ[3] += j2 * j0; JtJ[4] += j2 * j1; JtJ[5] += j2 * j2;
-        JtJ[6] += j3 * j0; JtJ[7] += j3 * j1; JtJ[8] += j3 * j2; JtJ[9] += j3 * j3;
-        gr[0] += j0 * r; gr[1] += j1 * r; gr[2] += j2 * r; gr[3] += j3 * r;
+        // S8(f)4: frame weights w_m (WLS; compiled out of the default path) -- J^T W J, J^T W r, 1/2 r^T W r
+        const double w = WLS ? fr[m].w : 1.0;
+        const double w0 = WLS ? w * j0 : j0, w1 = WLS ? w * j1 : j1, w2 = WLS ? w * j2 : j2, w3 = WLS ? w * j3 : j3;
+        phi += WLS ? 0.5 * (w * r) * r : 0.5 * r * r;
+        JtJ[0] += w0 * j0;
+        JtJ[1] += w1 * j0; JtJ[2] += w1 * j1;
+        JtJ[3] += w2 * j0; JtJ[4] += w2 * j1; JtJ[5] += w2 * j2;
+        JtJ[6] += w3 * j0; JtJ[7] += w3 * j1; JtJ[8] += w3 * j2; JtJ[9] += w3 * j3;
+        gr[0] += w0 * r; gr[1] += w1 * r; gr[2] += w2 * r; gr[3] += w3 * r;
     });
 #pragma unroll
     for (int q = 0; q < 10; ++q) out[q] = JtJ[q];
@@ -269,7 +273,9 @@ __device__ __forceinline__ void lm_eval(KKin kin, const KFrame *fr, const float 
 // 5 CTAs of 128 threads per SM (<= 102 registers): measured best of 1..8 on C2 and C4
 // TI / TO: storage type of the maps and of lambda on input / output.  Between the steps of one kcs_map_lm call the
 // iterate is kept in fp64 ping-pong buffers (TI = TO = double); only the caller's buffers are fp32.
-template <class TI, class TO>
+// OPT = false: the hot path of S8(a) (6 neighbours, one delta, unweighted).  OPT = true: the options of kcs_set_fit_options
+// (frame weights, nq = 6 or 10 neighbours, one delta per parameter), kept out of the default kernel's registers.
+template <class TI, class TO, bool OPT>
 #define KCS_LM_TPB 128
 #define KCS_LM_MINBLK 5
 // One thread per IN-MASK voxel: thread t of the launch fits voxel (z = t / M2, pixel vlist[t % M2]), M2 = in-mask pixels
@@ -278,8 +284,10 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
                                                  const TI *__restrict__ th_in, TO *__restrict__ th_out,
                                                  const TI *lam_in, TO *lam_out,  // may alias: each thread touches its own element
                                                  const unsigned char *__restrict__ mask, const int *__restrict__ vlist, int M2,
-                                                 long long nvox, double gamma, double delta, float *cost,
+                                                 long long nvox, double gamma, double4 delta4, int nq, float *cost,
                                                  double *__restrict__ st, long long nfit) {
+    constexpr int NQ = OPT ? 10 : 6;
+    constexpr bool WLS = OPT;
     // FIRST step of a call (fp32 input): the data part of the normal equations is evaluated at theta.  Later steps read
     // it from `st` [15][nfit], where the previous step left it for the iterate it produced: an accepted trial point was
     // evaluated WITH its Jacobian, a rejected step leaves theta -- and therefore J^T J, J^T r, Phi_data -- unchanged.
@@ -298,16 +306,21 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
     double xi[4];
 #pragma unroll
     for (int p = 0; p < 4; ++p) xi[p] = th_in[(size_t)p * nvox + v];
-    // Q13: in-volume, in-mask 6-neighbourhood of the previous iterate (Jacobi)
-    double nb[6][4];
+    // Q13: in-volume, in-mask 6-neighbourhood of the previous iterate (Jacobi); NQ = 10 (S8(f)2): the four in-plane
+    // diagonals of the 3x3 clique as well
+    const double delta[4] = {delta4.x, OPT ? delta4.y : delta4.x, OPT ? delta4.z : delta4.x, OPT ? delta4.w : delta4.x};
+    double nb[NQ][4];
     int nn = 0;
     {
-        const int di[6] = {-1, 1, 0, 0, 0, 0}, dj[6] = {0, 0, -1, 1, 0, 0}, dz[6] = {0, 0, 0, 0, -1, 1};
+        const int di[10] = {-1, 1, 0, 0, 0, 0, -1, 1, -1, 1}, dj[10] = {0, 0, -1, 1, 0, 0, -1, -1, 1, 1},
+                  dz[10] = {0, 0, 0, 0, -1, 1, 0, 0, 0, 0};
+        const int zr = z % g.nzr;  // slice index inside its replica
 #pragma unroll
-        for (int q = 0; q < 6; ++q) {
+        for (int q = 0; q < NQ; ++q) {
             const int ii = i + di[q], jj = j + dj[q], zz = z + dz[q];
-            const bool ok = ii >= 0 && ii < g.nx && jj >= 0 && jj < g.ny && zz >= 0 && zz < g.nz && zz / g.nzr == z / g.nzr &&
-                            mask[jj * g.nx + ii];  // in-volume, in the same replica, in-mask
+            // in-volume, in the same replica (slices [k nzr, (k+1) nzr)), in-mask
+            const bool zok = dz[q] == 0 || (dz[q] < 0 ? zr > 0 : zr < g.nzr - 1);
+            const bool ok = (!OPT || q < nq) && ii >= 0 && ii < g.nx && jj >= 0 && jj < g.ny && zok && mask[jj * g.nx + ii];
             if (ok) {
                 const size_t w = (size_t)zz * v2 + (size_t)jj * g.nx + ii;
 #pragma unroll
@@ -320,7 +333,7 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
 
     double ev[15];
     if (FIRST) {
-        lm_eval(kin, fr, x, xa.base, xa.fstride, xi[0], xi[1], xi[2], xi[3], ev);
+        lm_eval<WLS>(kin, fr, x, xa.base, xa.fstride, xi[0], xi[1], xi[2], xi[3], ev);
         if (!LAST) {
 #pragma unroll
             for (int q = 0; q < 15; ++q) st[(size_t)q * nfit + t] = ev[q];  // kept if this step is rejected
@@ -334,8 +347,8 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
             const double tt = xi[p] - nb[q][p];
-            phi_old += gamma * huber(tt, delta);
-            gr[p] -= gamma * huber_d(tt, delta);
+            phi_old += gamma * huber(tt, delta[p]);
+            gr[p] -= gamma * huber_d(tt, delta[p]);
         }
 
     double lam = lam_in[v];
@@ -353,11 +366,11 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
         double xt[4];
 #pragma unroll
         for (int p = 0; p < 4; ++p) xt[p] = fmin(fmax(xi[p] + d[p], lo[p]), hi[p]);
-        lm_eval(kin, fr, x, xa.base, xa.fstride, xt[0], xt[1], xt[2], xt[3], ev);
+        lm_eval<WLS>(kin, fr, x, xa.base, xa.fstride, xt[0], xt[1], xt[2], xt[3], ev);
         double phi_new = ev[14];
         for (int q = 0; q < nn; ++q)
 #pragma unroll
-            for (int p = 0; p < 4; ++p) phi_new += gamma * huber(xt[p] - nb[q][p], delta);
+            for (int p = 0; p < 4; ++p) phi_new += gamma * huber(xt[p] - nb[q][p], delta[p]);
         if (phi_new <= phi_old * (1.0 + 1e-6)) {  // Q15a: relative slack, see DESIGN.md section 3
 #pragma unroll
             for (int p = 0; p < 4; ++p) xi[p] = xt[p];
@@ -414,15 +427,20 @@ int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const vo
     if (nfit == 0) return KCS_OK;
     const unsigned grid = (unsigned)((nfit + KCS_LM_TPB - 1) / KCS_LM_TPB);
     ProfScope ps(c, KCS_K_LM);
-#define KCS_LM_GO(TI, TO)                                                                                              \
-    k_lm_step<TI, TO><<<grid, KCS_LM_TPB, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, (const TI *)theta_in, (TO *)theta_out, \
+    const double4 d4 = c->has_delta4 ? make_double4(c->delta4[0], c->delta4[1], c->delta4[2], c->delta4[3])
+                                     : make_double4((double)delta, (double)delta, (double)delta, (double)delta);
+    const bool opt = c->weighted || c->has_delta4 || c->nbr_mode != 6;
+#define KCS_LM_GO2(TI, TO, OPT)                                                                                        \
+    k_lm_step<TI, TO, OPT><<<grid, KCS_LM_TPB, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, (const TI *)theta_in, (TO *)theta_out, \
                                                        (const TI *)lam_in, (TO *)lam_out, c->d_mask, c->d_vlist, c->n_inmask2, nvox, (double)gamma,  \
-                                                       (double)delta, cost, c->lm_state, nfit)
+                                                       d4, c->nbr_mode, cost, c->lm_state, nfit)
+#define KCS_LM_GO(TI, TO) do { if (opt) KCS_LM_GO2(TI, TO, true); else KCS_LM_GO2(TI, TO, false); } while (0)
     if (!in_f64 && !out_f64) KCS_LM_GO(float, float);
     else if (!in_f64 && out_f64) KCS_LM_GO(float, double);
     else if (in_f64 && out_f64) KCS_LM_GO(double, double);
     else KCS_LM_GO(double, float);
 #undef KCS_LM_GO
+#undef KCS_LM_GO2
     LAUNCH_CHECK(c);
     return KCS_OK;
 }
