@@ -331,6 +331,7 @@ def time_config(torch, kcs, dev, name: str, steps: int, warmup: int) -> dict:
     ms = float(sum(a.elapsed_time(b) for a, b in evs))
     out = {"it_s": steps / ms * 1e3, "ms_per_iteration": ms / steps, "steps": steps, "warmup": warmup,
            "gpu_launches_per_iteration": (ctx.launch_count() - n0) / steps, "l2": run.l2_note,
+           "cuda_graph_replays": ctx.graph_replays(),
            "finite": bool(torch.isfinite(run.x).all() and torch.isfinite(run.th).all())}
     ctx.close()
     return out
@@ -372,6 +373,9 @@ def run_ours(args):
         raise SystemExit("bench.py: no CUDA device (this path has no CPU fallback)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    # everything runs on one non-default stream: the legacy default stream cannot be captured, and the launch-bound
+    # configurations (C1, C2) replay their iteration as a CUDA graph (kcs.h, kcs_use_graphs)
+    torch.cuda.set_stream(torch.cuda.Stream(device=dev))
     dist = None
     if world > 1:
         import torch.distributed as dist

@@ -85,6 +85,13 @@ int kcs_get_mask(const kcs_ctx *ctx, unsigned char *mask_host_out);
 /* Count of kernel launches this context has enqueued so far (bench.py's gpu_launches). */
 long long kcs_launch_count(const kcs_ctx *ctx);
 
+/* for launch-bound volumes (nz*ny*nx*T <= 4e6: C1, C2) kcs_icm_run / kcs_icm_iteration capture their kernel
+ * sequence into a CUDA graph on the first call with a given set of arguments and replay it afterwards (pointers and
+ * scalars are baked in, buffer contents are read at replay; results are bit-identical to the direct launches).
+ * kcs_use_graphs(ctx, 0) turns this off; kcs_graph_replays counts the replays so far. */
+int kcs_use_graphs(kcs_ctx *ctx, int on);
+long long kcs_graph_replays(const kcs_ctx *ctx);
+
 /* Optional per-kernel timing for the roofline report.  While enabled, every kernel launch of this
  * context is bracketed by CUDA events on the context's stream.  kcs_profile_read SYNCHRONISES the stream, adds the
  * elapsed milliseconds and launch counts since the previous read into ms[class] / count[class] ([host] arrays of
@@ -124,7 +131,9 @@ int kcs_osl_update(kcs_ctx *ctx, float *x, const float *bp, const float *sens, c
 
 /* K1-K6 (BJ configs[0](1)-(3)): frame-integrated model curve F[T][nz][ny][nx] and, if J != NULL,
  * its analytic Jacobian J[4][T][nz][ny][nx] from theta[4][nz][ny][nx].  Evaluated for every voxel (no mask).
- * Rate-dependent scalars are computed in fp64 on the device (fp32 cancels catastrophically). */
+ * Rate-dependent scalars are computed in fp64 on the device (fp32 cancels catastrophically).
+ * theta outside the box of Q16 is evaluated as given; for k2 + k3 = 0 (below the box: k2 >= 1e-4) F is the limit
+ * K1 (1 conv Cp) and dF/dk2, dF/dk3 are returned as 0. */
 int kcs_kinetic_eval(kcs_ctx *ctx, const float *theta, float *F, float *J);
 
 /* eq. 4-7 with readings L1-L3, Q12-Q16: n_steps synchronised (Jacobi) Levenberg-Marquardt

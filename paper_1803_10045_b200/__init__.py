@@ -31,7 +31,7 @@ PROFILE_CLASSES = ("pack", "unpack", "kinetic", "forward", "back", "lm", "other"
 
 # every symbol include/kcs.h declares (tests/test_abi.py checks the library exports each of them)
 EXPORTS = ["kcs_create", "kcs_destroy", "kcs_set_stream", "kcs_last_error", "kcs_workspace_bytes", "kcs_get_mask",
-           "kcs_launch_count", "kcs_profile_enable", "kcs_profile_read", "kcs_forward_project", "kcs_back_project", "kcs_sensitivity", "kcs_osl_update",
+           "kcs_launch_count", "kcs_use_graphs", "kcs_graph_replays", "kcs_profile_enable", "kcs_profile_read", "kcs_forward_project", "kcs_back_project", "kcs_sensitivity", "kcs_osl_update",
            "kcs_kinetic_eval", "kcs_ki_map", "kcs_set_multiplicative", "kcs_set_fit_options", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host"]
 
 
@@ -85,6 +85,9 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.kcs_launch_count.argtypes = [vp]
     lib.kcs_launch_count.restype = C.c_longlong
     lib.kcs_get_mask.argtypes = [vp, vp]
+    lib.kcs_use_graphs.argtypes = [vp, i]
+    lib.kcs_graph_replays.argtypes = [vp]
+    lib.kcs_graph_replays.restype = C.c_longlong
     lib.kcs_profile_enable.argtypes = [vp, i]
     lib.kcs_profile_read.argtypes = [vp, vp, vp, i]
     lib.kcs_forward_project.argtypes = [vp, fp, fp, i, i, i]
@@ -192,6 +195,12 @@ class Context:
 
     def launch_count(self) -> int:
         return int(self._lib.kcs_launch_count(self._h))
+
+    def use_graphs(self, on: bool = True):
+        self._check(self._lib.kcs_use_graphs(self._h, int(bool(on))))
+
+    def graph_replays(self) -> int:
+        return int(self._lib.kcs_graph_replays(self._h))
 
     def profile_enable(self, on: bool = True):
         self._check(self._lib.kcs_profile_enable(self._h, int(bool(on))))

@@ -174,6 +174,13 @@ int kcs_set_stream(kcs_ctx *ctx, void *stream) {
     return KCS_OK;
 }
 
+int kcs_use_graphs(kcs_ctx *c, int on) {
+    if (!c) return KCS_ERR_NULL;
+    c->use_graphs = on != 0;
+    return KCS_OK;
+}
+long long kcs_graph_replays(const kcs_ctx *ctx) { return ctx ? ctx->graph_replays : 0; }
+
 int kcs_profile_enable(kcs_ctx *c, int on) {
     if (!c) return KCS_ERR_NULL;
     c->prof_on = on != 0;
@@ -211,6 +218,7 @@ int kcs_destroy(kcs_ctx *c) {
                     c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->thD[0], c->thD[1], c->lamD, c->lm_state, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
     for (void *p : ptrs)
         if (p) cudaFree(p);
+    for (KGraphEntry &ge : c->graphs) cudaGraphExecDestroy(ge.exec);
     for (const KProfRec &r : c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
     if (c->in_stream) { cudaStreamDestroy(c->in_stream); cudaStreamDestroy(c->out_stream); cudaEventDestroy(c->ev_small); }
@@ -243,6 +251,9 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->stream = (cudaStream_t)stream;
     c->launches = 0;
     c->ws_bytes = 0;
+    c->use_graphs = true;
+    c->opt_gen = 0;
+    c->graph_replays = 0;
     c->prof_on = false;
     c->xi_border_tp = 0;
     c->d_fwd = c->d_bwd = nullptr; c->d_frames = nullptr; c->d_mask = nullptr;
@@ -440,6 +451,7 @@ int kcs_sensitivity(kcs_ctx *c, int subset, float *sens) {
 // S8(f)3: the sensitivity images A_s^T n are one plain back-projection of n (as a one-frame sinogram) per subset.
 int kcs_set_multiplicative(kcs_ctx *c, const float *mult) {
     if (!c) return KCS_ERR_NULL;
+    c->opt_gen++;
     const KGeom &g = c->g;
     if (!mult) {  // back to unit factors
         if (c->d_mult) { cudaStreamSynchronize(c->stream); cudaFree(c->d_mult); c->d_mult = nullptr; }
@@ -528,6 +540,7 @@ int kcs_set_fit_options(kcs_ctx *c, const double *frame_weights, int neighbourho
         if (frame_weights && !(frame_weights[m] >= 0.0)) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: negative frame weight");
     for (int p = 0; p < 4; ++p)
         if (delta4 && !(delta4[p] >= 0.0)) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: negative delta");
+    c->opt_gen++;
     c->weighted = false;
     for (int m = 0; m < T; ++m) {
         c->h_frames[m].w = frame_weights ? frame_weights[m] : 1.0;
@@ -656,9 +669,85 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
     return KCS_OK;
 }
 
+// S:7-H6.  A small problem's ICM iteration is ~20 kernels of a few microseconds each: launch-bound.  The first
+// kcs_icm_run with a given set of arguments is CAPTURED into a CUDA graph (the second-stream fork / join included) and
+// launched; later calls with the same arguments replay it with one cudaGraphLaunch.  The graph bakes in pointers and
+// scalars only -- buffer CONTENTS are read at replay time -- and is dropped when an option it depends on changes.
+// Not used while per-kernel profiling is on, when the caller's stream is itself being captured, or for volumes that
+// are not launch-bound.
+static bool graph_eligible(kcs_ctx *c, int n_iter) {
+    if (!c->use_graphs || c->prof_on || n_iter <= 0 || n_iter > 16) return false;
+    if ((double)c->n_vox * c->cfg.n_frames > 4.0e6) return false;  // C1, C2-sized; C3 and C4 keep the GPU busy per launch
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(c->stream, &st) != cudaSuccess || st != cudaStreamCaptureStatusNone) { cudaGetLastError(); return false; }
+    return true;
+}
+
 int kcs_icm_run(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta, float *lambda,
                 float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter) {
-    return icm_run_impl(c, y, r, r_mode, scale, x, theta, lambda, beta_first, beta, gamma, delta, n_lm, n_iter, nullptr);
+    if (!c) return KCS_ERR_NULL;
+    if (!y || !r || !x || !theta || !lambda || (r_mode != KCS_R_PER_FRAME && r_mode != KCS_R_FULL) || n_lm < 0 || !(scale > 0.f) ||
+        !graph_eligible(c, n_iter))
+        return icm_run_impl(c, y, r, r_mode, scale, x, theta, lambda, beta_first, beta, gamma, delta, n_lm, n_iter, nullptr);
+    for (size_t q = 0; q < c->graphs.size(); ++q) {
+        const KGraphEntry &ge = c->graphs[q];
+        if (ge.y == y && ge.r == r && ge.x == x && ge.theta == theta && ge.lambda == lambda && ge.r_mode == r_mode &&
+            ge.n_lm == n_lm && ge.n_iter == n_iter && ge.scale == scale && ge.beta_first == beta_first && ge.beta == beta &&
+            ge.gamma == gamma && ge.delta == delta && ge.stream == c->stream && ge.gen == c->opt_gen) {
+            // an intervening call with another frame count may have left xi with another layout: the border must be valid
+            int rc = ensure_border(c, round_up4(c->cfg.n_frames));
+            if (rc) return rc;
+            KCS_CUDA_OK(c, cudaGraphLaunch(ge.exec, c->stream));
+            c->launches += ge.launches;
+            c->graph_replays++;
+            return KCS_OK;
+        }
+    }
+    // everything that may not happen during capture happens now: allocations, stream / event creation, the border memset
+    const int Tp = round_up4(c->cfg.n_frames);
+    int rc = ensure_border(c, Tp);
+    if (rc) return rc;
+    if (r_mode == KCS_R_FULL && !c->ri && dalloc(c, &c->ri, c->n_ray_all * Tp) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, KCS_ERR_ALLOC, "kcs_icm: cannot allocate the packed randoms sinogram");
+    }
+    if (!c->aux_stream) {
+        KCS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+    }
+    const long long n0 = c->launches;
+    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        return icm_run_impl(c, y, r, r_mode, scale, x, theta, lambda, beta_first, beta, gamma, delta, n_lm, n_iter, nullptr);
+    }
+    rc = icm_run_impl(c, y, r, r_mode, scale, x, theta, lambda, beta_first, beta, gamma, delta, n_lm, n_iter, nullptr);
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (rc != KCS_OK || e != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        if (rc != KCS_OK) return rc;
+        c->launches = n0;  // capture failed: run the call directly
+        return icm_run_impl(c, y, r, r_mode, scale, x, theta, lambda, beta_first, beta, gamma, delta, n_lm, n_iter, nullptr);
+    }
+    KGraphEntry ge{y, r, x, theta, lambda, r_mode, n_lm, n_iter, scale, beta_first, beta, gamma, delta, c->stream, c->opt_gen,
+                   c->launches - n0, nullptr};
+    e = cudaGraphInstantiate(&ge.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        c->launches = n0;
+        return icm_run_impl(c, y, r, r_mode, scale, x, theta, lambda, beta_first, beta, gamma, delta, n_lm, n_iter, nullptr);
+    }
+    // keep the graphs of the current option generation only, at most 8 of them
+    for (size_t q = 0; q < c->graphs.size();) {
+        if (c->graphs[q].gen != c->opt_gen || c->graphs.size() >= 8) { cudaGraphExecDestroy(c->graphs[q].exec); c->graphs.erase(c->graphs.begin() + q); }
+        else ++q;
+    }
+    c->graphs.push_back(ge);
+    KCS_CUDA_OK(c, cudaGraphLaunch(ge.exec, c->stream));
+    return KCS_OK;
 }
 
 int kcs_icm_iteration(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta,

@@ -64,6 +64,17 @@ struct KProfRec {
     int cls;
 };
 
+// A captured kcs_icm_run call (S:7-H6: small problems are launch-bound; a replay is one cudaGraphLaunch).
+struct KGraphEntry {
+    const void *y, *r, *x, *theta, *lambda;
+    int r_mode, n_lm, n_iter;
+    float scale, beta_first, beta, gamma, delta;
+    cudaStream_t stream;
+    long long gen;          // option generation of the context when it was captured
+    long long launches;     // kernels inside
+    cudaGraphExec_t exec;
+};
+
 struct kcs_ctx {
     kcs_config cfg;
     bool prof_on;
@@ -74,6 +85,9 @@ struct kcs_ctx {
     std::string err;
     long long launches;
     long long ws_bytes;
+    bool use_graphs;                    // kcs_use_graphs (default on)
+    long long opt_gen, graph_replays;   // bumped by every call that changes what a captured graph bakes in
+    std::vector<KGraphEntry> graphs;
 
     KGeom g;
     KKin kin;
