@@ -121,15 +121,15 @@ struct FwdArgs {
 };
 
 #define KCS_ANCHOR 16  // steps between fp64 re-anchoring of the sample coordinates
-#define KCS_FWD_UNROLL 4
+#define KCS_FWD_UNROLL 2  // x 6 CTAs per SM: 3.02 ms per C4 subset launch; 1..8 x 1..8 CTAs all land within 4 % (3.02-3.13), 8 x 1: 3.62
 #define KCS_FWD_TPB 128
 #define KCS_BACK_TPB 128  // 4 CTAs of 128 threads per SM (128 registers): 2.64 ms per C4 subset launch against 2.71 with 2 x 256
 
 // One thread = one ray x 4 frames; the FG = Tp/4 lanes of a ray read a whole pixel (16 FG bytes) per tap in one request.
 template <int FG>
-__global__ void __launch_bounds__(KCS_FWD_TPB, 1) k_forward(KGeom g, FwdArgs p) {
+__global__ void __launch_bounds__(KCS_FWD_TPB, 6) k_forward(KGeom g, FwdArgs p) {
     constexpr int FPT = 4, Tp = 4 * FG;
-    // 16 loads in flight per thread pay when a warp covers few rays (FG >= 4); with 16-32 rays per warp the extra
+    // 8 loads in flight per thread when a warp covers few rays (FG >= 4); with 16-32 rays per warp the extra
     // registers cost more occupancy than the unrolling hides (C5(a) at 1 and 4 frames per launch)
     constexpr int kUnroll = FG >= 4 ? KCS_FWD_UNROLL : 1;
     extern __shared__ float red[];
