@@ -434,8 +434,13 @@ int kcs_launch_build_wtab(kcs_ctx *c) {
 // the window's 5 sinogram values are loaded once (5 LDG.128, one 128 B line each at Tp = 32) and serve all four
 // voxels: 1.25 L1 wavefronts per voxel-angle instead of 3.  Weights come from the k_build_wtab table (L2 resident:
 // it is the same for every slice and frame).  No atomics: run-to-run deterministic.
-template <int ZB>
-__global__ void __launch_bounds__(KCS_BACK_TPB, 4) k_back(KGeom g, BackArgs p) {
+// Two instantiations are used (round 2, C4, per subset launch; results are bit-identical):
+//   <2, true>   two slices per thread, the record of angle l+1 requested before the math of angle l, 4 CTAs per SM: the
+//               plain back-projection (all 252 angles: 47.7 ms against 54.3);
+//   <1, false>  one slice per thread, no prefetch, 80 registers, 6 CTAs per SM: the fused OSL update, whose epilogue
+//               (x and F from HBM) overlaps other CTAs' angle loops better at 24 warps per SM (2.50 ms against 2.64).
+template <int ZB, bool PIPE>
+__global__ void __launch_bounds__(KCS_BACK_TPB, PIPE ? 4 : 6) k_back(KGeom g, BackArgs p) {
     const int tid = threadIdx.x;
     const int fg = tid % p.FG;
     const int blk = tid / p.FG;
@@ -484,11 +489,15 @@ __global__ void __launch_bounds__(KCS_BACK_TPB, 4) k_back(KGeom g, BackArgs p) {
         // slices of an angle are requested together, so a thread waits on global memory once per angle, not ZB+1 times
         // (ncu source page of the un-pipelined loop: 16 % of the stall samples on the record, 4 x 5.5 % on the windows).
         float4 n0, n1, n2, n3, n4, n5;
-        {
+        if (PIPE) {
             const float4 *rec = rec0 + (size_t)(p.subset < 0 ? 0 : p.subset) * astride;
             n0 = __ldg(rec); n1 = __ldg(rec + 4); n2 = __ldg(rec + 8); n3 = __ldg(rec + 12); n4 = __ldg(rec + 16); n5 = __ldg(rec + 20);
         }
         for (int l = 0; l < p.As; ++l) {
+            if (!PIPE) {
+                const float4 *rec = rec0 + (size_t)(p.subset < 0 ? l : p.subset + l * g.S) * astride;
+                n0 = __ldg(rec); n1 = __ldg(rec + 4); n2 = __ldg(rec + 8); n3 = __ldg(rec + 12); n4 = __ldg(rec + 16); n5 = __ldg(rec + 20);
+            }
             const float4 r0 = n0, r1 = n1, r2 = n2, r3 = n3, r4 = n4, r5 = n5;
             const int base = __float_as_int(r0.x);
             float4 q[ZB][5];
@@ -499,7 +508,7 @@ __global__ void __launch_bounds__(KCS_BACK_TPB, 4) k_back(KGeom g, BackArgs p) {
 #pragma unroll
                 for (int r = 0; r < 5; ++r) q[zb][r] = __ldg(reinterpret_cast<const float4 *>(row + r * Tp));
             }
-            if (l + 1 < p.As) {
+            if (PIPE && l + 1 < p.As) {
                 const float4 *rec = rec0 + (size_t)(p.subset < 0 ? l + 1 : p.subset + (l + 1) * g.S) * astride;
                 n0 = __ldg(rec); n1 = __ldg(rec + 4); n2 = __ldg(rec + 8); n3 = __ldg(rec + 12); n4 = __ldg(rec + 16); n5 = __ldg(rec + 20);
             }
@@ -616,15 +625,14 @@ int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, f
     p.BX = nblk >= 128 ? 16 : 8;
     p.BY = nblk / p.BX;
     const int gx = (g.nx + 2 * p.BX - 1) / (2 * p.BX), gy = (g.ny + 2 * p.BY - 1) / (2 * p.BY);
+    // plain back-projection: two slices per thread when that still fills the GPU; fused OSL update: one (see k_back)
     int ZB = 1;
-    // ZB <= 2: the pipelined loop keeps the windows of all ZB slices (and the epilogue their x and F lines) in registers
-    if (g.nz >= 2 && (long long)gx * gy * ((g.nz + 1) / 2) >= 148LL) ZB = 2;
+    if (!osl && g.nz >= 2 && (long long)gx * gy * ((g.nz + 1) / 2) >= 148LL) ZB = 2;
     dim3 grid(gx, gy, (g.nz + ZB - 1) / ZB);
     ProfScope ps(c, KCS_K_BACK);
-    switch (ZB) {
-        case 2: k_back<2><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p); break;
-        default: k_back<1><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p); break;
-    }
+    if (osl) k_back<1, false><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
+    else if (ZB == 2) k_back<2, true><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
+    else k_back<1, true><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
     LAUNCH_CHECK(c);
     return KCS_OK;
 }
