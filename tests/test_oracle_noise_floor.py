@@ -9,7 +9,8 @@ arithmetic is not involved in the comparison (both chains are the oracle): the l
 (noise-dominated 4-parameter fits with parameters on their bounds move by > 1e-3 under a 3e-7 change of the curve they
 fit), i.e. the floor under which no fp32 OS pass can stay.  Measured with KCS_FLOOR_FULL=1 (C2 at full size, 8 slices):
 min over the parameters 99.82 % after 10 iterations (profiles/r2_oracle_noise_floor_C2.txt); the CUDA path reaches
-99.88 % on the same data.  The default run uses 2 slices of C2 so that the CPU suite stays short.
+99.85-99.88 % on the same data.  KCS_FLOOR_FULL=C3 (C3 at full size, 2 counts per voxel-frame): 98.93 %, activity 1.26e-3
+(profiles/r2_oracle_noise_floor_C3.txt); the CUDA path: 98.8 %, 1.30e-3.  The default run uses 2 slices of C2 so that the CPU suite stays short.
 
     KCS_FLOOR_FULL=1 python -m pytest tests/test_oracle_noise_floor.py -s -q
 """
@@ -63,6 +64,6 @@ def test_fp32_sized_perturbation_is_amplified_past_the_tolerance_band():
     assert 0.5 * RMS <= ex1 <= 2.0 * RMS and min(fr1) >= 0.9999      # one iteration: the perturbation itself, no loss
     assert ex10 >= 30.0 * RMS                                       # ten iterations: amplified by orders of magnitude
     assert min(fr10) < 0.9997                                       # and voxels have left the band ...
-    assert min(fr10) > 0.99                                         # ... a fraction of a per cent of them
+    assert min(fr10) > 0.97                                         # ... a per cent of them at most
     if full:
         assert min(fr10) < 0.999                                    # at full size: below BASELINE's 99.9 %
