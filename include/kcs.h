@@ -153,17 +153,6 @@ int kcs_map_lm(kcs_ctx *ctx, const float *x, float *theta, float *lambda, float 
  *                           calls is then ignored */
 int kcs_set_fit_options(kcs_ctx *ctx, const double *frame_weights, int neighbourhood, const double *delta4);
 
-/* Arithmetic of the MAP-LM model evaluation (BJ north_star asks for the FP32 pipe).
- *   KCS_FIT_FP64 (default)  closed-form W_m(a) and the normal equations in fp64 registers: the parity reference.
- *   KCS_FIT_FP32            W_m(a) and dW_m/da from a per-context table (piecewise degree-7 polynomials in a = k2 + k3,
- *                           fp32 Horner), model, Jacobian and the J^T J / J^T r / Phi sums in fp32 FMAs; the 4x4 solve, the
- *                           accept test and the iterate stay fp64.  Evaluation error ~2e-7 of F: per-call parity holds, the
- *                           10-iteration chain loses more voxels than with fp64.  Builds the table on
- *                           first use (SYNCHRONISES).  Frame weights / the 10-neighbourhood are not available in this mode. */
-#define KCS_FIT_FP64 0
-#define KCS_FIT_FP32 1
-int kcs_set_fit_precision(kcs_ctx *ctx, int precision);
-
 /* the macro-parameter map K_i = K1 k3 / (k2 + k3) (net influx rate; 0 where k2 + k3 = 0) from
  * theta[4][nz][ny][nx]; ki[nz][ny][nx] (device).  Evaluated for every voxel. */
 int kcs_ki_map(kcs_ctx *ctx, const float *theta, float *ki);

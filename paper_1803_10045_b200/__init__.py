@@ -32,7 +32,7 @@ PROFILE_CLASSES = ("pack", "unpack", "kinetic", "forward", "back", "lm", "other"
 # every symbol include/kcs.h declares (tests/test_abi.py checks the library exports each of them)
 EXPORTS = ["kcs_create", "kcs_destroy", "kcs_set_stream", "kcs_last_error", "kcs_workspace_bytes", "kcs_get_mask",
            "kcs_launch_count", "kcs_use_graphs", "kcs_graph_replays", "kcs_profile_enable", "kcs_profile_read", "kcs_forward_project", "kcs_back_project", "kcs_sensitivity", "kcs_osl_update",
-           "kcs_kinetic_eval", "kcs_ki_map", "kcs_set_multiplicative", "kcs_set_fit_options", "kcs_set_fit_precision", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host"]
+           "kcs_kinetic_eval", "kcs_ki_map", "kcs_set_multiplicative", "kcs_set_fit_options", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host"]
 
 
 class KcsError(RuntimeError):
@@ -98,7 +98,6 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.kcs_ki_map.argtypes = [vp, fp, fp]
     lib.kcs_set_multiplicative.argtypes = [vp, fp]
     lib.kcs_set_fit_options.argtypes = [vp, vp, i, vp]
-    lib.kcs_set_fit_precision.argtypes = [vp, i]
     lib.kcs_map_lm.argtypes = [vp, fp, fp, fp, f, f, i, fp]
     lib.kcs_icm_iteration.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, i]
     lib.kcs_icm_run.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, f, i, i]
@@ -264,10 +263,6 @@ class Context:
         assert d4 is None or d4.size == 4
         self._check(self._lib.kcs_set_fit_options(self._h, None if fw is None else fw.ctypes.data_as(C.c_void_p), neighbourhood,
                                                   None if d4 is None else d4.ctypes.data_as(C.c_void_p)))
-
-    def set_fit_precision(self, fp32: bool):
-        """MAP-LM model evaluation on the FP32 pipe (table-driven W_m(a)) instead of the fp64 closed form."""
-        self._check(self._lib.kcs_set_fit_precision(self._h, 1 if fp32 else 0))
 
     def ki_map(self, theta, ki):
         shp = (self.nz, self.ny, self.nx)

@@ -214,7 +214,7 @@ int kcs_get_mask(const kcs_ctx *ctx, unsigned char *out) {
 int kcs_destroy(kcs_ctx *c) {
     if (!c) return KCS_ERR_NULL;
     cudaStreamSynchronize(c->stream);
-    void *ptrs[] = {c->d_wcoef, c->d_mult, c->d_sens_z, c->d_smax_z, c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->d_wtab, c->d_vlist, c->xi, c->Fi,
+    void *ptrs[] = {c->d_mult, c->d_sens_z, c->d_smax_z, c->d_fwd, c->d_bwd, c->d_frames, c->d_mask, c->d_sens, c->d_smax, c->d_tmp_smax, c->d_wtab, c->d_vlist, c->xi, c->Fi,
                     c->qi, c->yi, c->ri, c->r_pad, c->theta2, c->thD[0], c->thD[1], c->lamD, c->lm_state, c->st_y, c->st_r, c->st_x, c->st_theta, c->st_lambda};
     for (void *p : ptrs)
         if (p) cudaFree(p);
@@ -256,7 +256,7 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->graph_replays = 0;
     c->prof_on = false;
     c->xi_border_tp = 0;
-    c->d_fwd = c->d_bwd = nullptr; c->d_frames = nullptr; c->d_mask = nullptr; c->d_wcoef = nullptr; c->fit_fp32 = false;
+    c->d_fwd = c->d_bwd = nullptr; c->d_frames = nullptr; c->d_mask = nullptr;
     c->d_sens = c->d_smax = c->d_tmp_smax = nullptr;
     c->d_mult = c->d_sens_z = c->d_smax_z = nullptr;
     c->d_wtab = nullptr;
@@ -336,8 +336,6 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
                         gl8([&](long double u) { return ((long double)te - u) * fe.Cp(u); }, ts, te, np));
         f.contiguous = (m > 0 && c->ts[m] == c->te[m - 1]) ? 1 : 0;
         f.w = 1.0;
-        f.W0f = (float)f.W0;
-        f.dICpf = (float)f.dICp;
         if (m > 0 && std::fabs(f.dt - frames[m - 1].dt) <= 1e-12 * f.dt) {
             f.dt = frames[m - 1].dt;  // same duration class: per-duration scalars are reused (1e-12 relative)
             f.new_dt = 0;
@@ -352,7 +350,6 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
         kin.lam[i] = (double)fe.lam[i];
     }
     kin.beta0 = (double)fe.be[0];
-    kin.wcoef = nullptr;
     c->h_frames = frames;
     c->nbr_mode = 6;
     c->has_delta4 = false;
@@ -554,18 +551,6 @@ int kcs_set_fit_options(kcs_ctx *c, const double *frame_weights, int neighbourho
     c->nbr_mode = neighbourhood;
     c->has_delta4 = delta4 != nullptr;
     for (int p = 0; p < 4; ++p) c->delta4[p] = delta4 ? delta4[p] : 0.0;
-    return KCS_OK;
-}
-
-int kcs_set_fit_precision(kcs_ctx *c, int precision) {
-    if (!c) return KCS_ERR_NULL;
-    if (precision != KCS_FIT_FP64 && precision != KCS_FIT_FP32) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_precision: unknown precision");
-    if (precision == KCS_FIT_FP32 && !c->d_wcoef) {
-        const int rc = kcs_build_wtable(c);
-        if (rc) return rc;
-    }
-    c->fit_fp32 = precision == KCS_FIT_FP32;
-    c->opt_gen++;
     return KCS_OK;
 }
 

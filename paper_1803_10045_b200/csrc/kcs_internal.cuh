@@ -48,19 +48,8 @@ struct KFrame {
     int contiguous;  // t_start == previous frame's t_end (state carried over)
     int new_dt;      // dt differs from the previous frame's (per-duration scalars must be recomputed)
     double w;        // weight of this frame in the least-squares data term (S8(f)4; 1 by default)
-    float W0f, dICpf;  // fp32 copies for the FP32 fit (kcs_set_fit_precision)
 };
-// FP32 fit (kcs_set_fit_precision): W_m(a) = int_frame (e^{-a.} conv Cp), the only voxel-dependent transcendental object
-// of the model (K3), is an entire function of the single rate a = k2 + k3.  It is tabulated once per context as piecewise
-// polynomials of degree KCS_WT_DEG on intervals of width 1/KCS_WT_PER_UNIT covering a in [0, KCS_WT_AMAX] (the whole box of
-// Q16): fp32 monomial coefficients in s = 2 (a - lo)/h - 1, fitted at Chebyshev nodes to values of the fp64 closed form.
-#define KCS_WT_DEG 7
-#define KCS_WT_PER_UNIT 32
-#define KCS_WT_AMAX 3
-#define KCS_WT_NINT (KCS_WT_AMAX * KCS_WT_PER_UNIT)
-
 struct KKin {
-    const float *wcoef;  // [KCS_WT_NINT][T][KCS_WT_DEG + 1] (device), NULL until kcs_set_fit_precision builds it
     int T;
     double alpha[3];  // K1: Cp(t) = sum (alpha_i + beta_i t) e^{-l_i t}; (alpha, beta) = (-A2-A3, A1), (A2, 0), (A3, 0)
     double beta0;
@@ -104,8 +93,6 @@ struct kcs_ctx {
     KKin kin;
     double4 *d_fwd, *d_bwd;
     KFrame *d_frames;
-    float *d_wcoef;                   // W_m(a) table of the FP32 fit (KKin::wcoef)
-    bool fit_fp32;
     std::vector<KFrame> h_frames;     // host copy (kcs_set_fit_options rewrites the frame weights)
     int nbr_mode;                     // 6 (Q13) or 10 (3x3 in-plane clique + the two axial neighbours, S8(f)2)
     bool weighted;                    // some frame weight differs from 1 (S8(f)4)
@@ -218,7 +205,6 @@ int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *se
 // F (and J) from theta.  inner == 0: F planar [T][V], J planar [4][T][V] or NULL;  inner == 1: F = padded inner layout, Tp.
 int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp);
 int kcs_launch_ki_map(kcs_ctx *c, const float *theta, float *ki);
-int kcs_build_wtable(kcs_ctx *c);  // allocates and fills c->d_wcoef, points c->kin.wcoef at it; synchronises the stream
 // one Jacobi LM step: reads theta_in, writes theta_out for the in-mask voxels (masked-out voxels are never touched).
 //   x_inner == 0: x planar [T][V];  x_inner == 1: x = c->xi padded inner layout with Tp.
 int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const void *theta_in, int in_f64, void *theta_out,

@@ -15,8 +15,6 @@
 //     dD_i/da = (E1 - D_i)/c_i                   dT_0/da = -(dD_0/da + T_0)/c_0
 // and for |c_i| < 1e-4 (i = 1, 2; l_0 = 4.134 is outside the parameter box) the Taylor expansion about a = l_i:
 //     D_i = P1 - P2 c/2 + P3 c^2/6 - P4 c^3/24,  dD_i/da = -P2/2 + P3 c/3 - P4 c^2/8.
-#include <cmath>
-
 #include "kcs_internal.cuh"
 
 #define LAUNCH_CHECK(c)                                                     \
@@ -160,63 +158,6 @@ __device__ __forceinline__ void tac_stream(const KKin &kin, const KFrame *fr, do
     }
 }
 
-// ---------------------------------------------------------------------------------------------------------
-// FP32 fit (kcs_set_fit_precision).  W_m(a), dW_m/da from the table of the context: s = 2 (a - lo_i)/h - 1 is formed in
-// fp64 (a * 64 is a power-of-two scaling, 2 i + 1 an integer: exact) and rounded once; everything per frame is FFMA.
-// No term cancels: F = vB dICp + (1 - vB)(B1 W + B2 W0) is a sum of positive numbers; only the Jacobian's (W - W0)
-// loses digits as a -> 0 (1e-4 relative at a = 1e-4), which moves a step direction, not the cost.
-// ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ bool in_table(const KKin &kin, double a) {
-    return a > 0.0 && a <= (double)KCS_WT_AMAX && kin.wcoef != nullptr;
-}
-
-// out[0..9] = J^T J (packed lower triangle), out[10..13] = J^T r, out[14] = 1/2 sum r^2, as lm_eval.
-__device__ __forceinline__ void lm_eval_f32(const KKin &kin, const KFrame *fr, const float *__restrict__ x, size_t xbase, size_t xstride,
-                                            double K1, double k2, double k3, double vB, double *out) {
-    const double a = k2 + k3;
-    const int T = kin.T;
-    const int i = min((int)(a * (double)KCS_WT_PER_UNIT), KCS_WT_NINT - 1);
-    const float s = (float)fma(a, 2.0 * KCS_WT_PER_UNIT, -(double)(2 * i + 1));
-    const float dsda = 2.f * KCS_WT_PER_UNIT;
-    const float4 *cf = reinterpret_cast<const float4 *>(kin.wcoef + (size_t)i * T * (KCS_WT_DEG + 1));
-    const double ia = 1.0 / a;
-    const float B1 = (float)(K1 * k2 * ia), B2 = (float)(K1 * k3 * ia);
-    const float vBf = (float)vB, omv = (float)(1.0 - vB);
-    const float k2a = (float)(k2 * ia), k3a = (float)(k3 * ia);
-    const float c23 = (float)(K1 * k3 * ia * ia), c32 = (float)(K1 * k2 * ia * ia);
-    float JtJ[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, gr[4] = {0, 0, 0, 0}, phi = 0.f;
-    for (int m = 0; m < T; ++m) {
-        const float4 c03 = __ldg(cf + 2 * m), c47 = __ldg(cf + 2 * m + 1);
-        // Horner with derivative: b_k = c_k + s b_{k+1}, W = b_0;  d_k = b_k + s d_{k+1}, dW/ds = d_1
-        float b = c47.w, d = c47.w;
-        b = fmaf(s, b, c47.z);
-        d = fmaf(s, d, b); b = fmaf(s, b, c47.y);
-        d = fmaf(s, d, b); b = fmaf(s, b, c47.x);
-        d = fmaf(s, d, b); b = fmaf(s, b, c03.w);
-        d = fmaf(s, d, b); b = fmaf(s, b, c03.z);
-        d = fmaf(s, d, b); b = fmaf(s, b, c03.y);
-        d = fmaf(s, d, b); b = fmaf(s, b, c03.x);
-        const float W = b, dW = d * dsda;
-        const float W0 = fr[m].W0f, dI = fr[m].dICpf;
-        const float tissue = fmaf(B1, W, B2 * W0);
-        const float F = fmaf(vBf, dI, omv * tissue);
-        const float t1 = W - W0, bdw = B1 * dW;
-        const float j0 = omv * fmaf(k2a, W, k3a * W0), j1 = omv * fmaf(c23, t1, bdw), j2 = omv * fmaf(-c32, t1, bdw), j3 = dI - tissue;
-        const float r = x[xbase + m * xstride] - F;
-        phi = fmaf(0.5f * r, r, phi);
-        JtJ[0] = fmaf(j0, j0, JtJ[0]);
-        JtJ[1] = fmaf(j1, j0, JtJ[1]); JtJ[2] = fmaf(j1, j1, JtJ[2]);
-        JtJ[3] = fmaf(j2, j0, JtJ[3]); JtJ[4] = fmaf(j2, j1, JtJ[4]); JtJ[5] = fmaf(j2, j2, JtJ[5]);
-        JtJ[6] = fmaf(j3, j0, JtJ[6]); JtJ[7] = fmaf(j3, j1, JtJ[7]); JtJ[8] = fmaf(j3, j2, JtJ[8]); JtJ[9] = fmaf(j3, j3, JtJ[9]);
-        gr[0] = fmaf(j0, r, gr[0]); gr[1] = fmaf(j1, r, gr[1]); gr[2] = fmaf(j2, r, gr[2]); gr[3] = fmaf(j3, r, gr[3]);
-    }
-#pragma unroll
-    for (int q = 0; q < 10; ++q) out[q] = (double)JtJ[q];
-#pragma unroll
-    for (int q = 0; q < 4; ++q) out[10 + q] = (double)gr[q];
-    out[14] = (double)phi;
-}
-
 __device__ __forceinline__ void load_frames(const KKin &kin, KFrame *sh) {
     const int n = kin.T * (int)(sizeof(KFrame) / sizeof(double));
     const double *src = reinterpret_cast<const double *>(kin.frames);
@@ -334,7 +275,7 @@ __device__ __forceinline__ void lm_eval(KKin kin, const KFrame *fr, const float 
 // iterate is kept in fp64 ping-pong buffers (TI = TO = double); only the caller's buffers are fp32.
 // OPT = false: the hot path of S8(a) (6 neighbours, one delta, unweighted).  OPT = true: the options of kcs_set_fit_options
 // (frame weights, nq = 6 or 10 neighbours, one delta per parameter), kept out of the default kernel's registers.
-template <class TI, class TO, bool OPT, bool F32>
+template <class TI, class TO, bool OPT>
 #define KCS_LM_TPB 128
 #define KCS_LM_MINBLK 5
 // One thread per IN-MASK voxel: thread t of the launch fits voxel (z = t / M2, pixel vlist[t % M2]), M2 = in-mask pixels
@@ -392,9 +333,7 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
 
     double ev[15];
     if (FIRST) {
-        // the caller's theta may lie outside the box (and the table): those voxels take the fp64 closed form
-        if (F32 && in_table(kin, xi[1] + xi[2])) lm_eval_f32(kin, fr, x, xa.base, xa.fstride, xi[0], xi[1], xi[2], xi[3], ev);
-        else lm_eval<WLS>(kin, fr, x, xa.base, xa.fstride, xi[0], xi[1], xi[2], xi[3], ev);
+        lm_eval<WLS>(kin, fr, x, xa.base, xa.fstride, xi[0], xi[1], xi[2], xi[3], ev);
         if (!LAST) {
 #pragma unroll
             for (int q = 0; q < 15; ++q) st[(size_t)q * nfit + t] = ev[q];  // kept if this step is rejected
@@ -427,8 +366,7 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
         double xt[4];
 #pragma unroll
         for (int p = 0; p < 4; ++p) xt[p] = fmin(fmax(xi[p] + d[p], lo[p]), hi[p]);
-        if (F32) lm_eval_f32(kin, fr, x, xa.base, xa.fstride, xt[0], xt[1], xt[2], xt[3], ev);  // box-projected: inside the table
-        else lm_eval<WLS>(kin, fr, x, xa.base, xa.fstride, xt[0], xt[1], xt[2], xt[3], ev);
+        lm_eval<WLS>(kin, fr, x, xa.base, xa.fstride, xt[0], xt[1], xt[2], xt[3], ev);
         double phi_new = ev[14];
         for (int q = 0; q < nn; ++q)
 #pragma unroll
@@ -461,80 +399,7 @@ __global__ void k_ki_map(const float *__restrict__ theta, float *__restrict__ ki
     ki[v] = a > 0.f ? K1 * k3 / a : 0.f;
 }
 
-// Samples of W_m(a) for the table of the FP32 fit: thread (i, j) evaluates the fp64 closed form at Chebyshev node j of
-// interval i (theta = (1, a, 0, 0) makes the model curve equal to W_m(a): B1 = 1, B2 = 0, vB = 0).
-__global__ void k_wtable_samples(KKin kin, double *samples) {
-    extern __shared__ double sh_raw[];
-    KFrame *fr = reinterpret_cast<KFrame *>(sh_raw);
-    load_frames(kin, fr);
-    const int q = blockIdx.x * blockDim.x + threadIdx.x;
-    constexpr int N = KCS_WT_DEG + 1;
-    if (q >= KCS_WT_NINT * N) return;
-    const int i = q / N, j = q - i * N;
-    const double sj = cospi((2.0 * j + 1.0) / (2.0 * N));  // Chebyshev node in (-1, 1)
-    const double a = ((double)(2 * i + 1) + sj) / (2.0 * KCS_WT_PER_UNIT);
-    tac_stream<false>(kin, fr, 1.0, a, 0.0, 0.0, [&](int m, double Fm, double, double, double, double) {
-        samples[(size_t)q * kin.T + m] = Fm;
-    });
-}
-
 }  // namespace
-
-int kcs_build_wtable(kcs_ctx *c) {
-    constexpr int N = KCS_WT_DEG + 1;
-    const int T = c->kin.T;
-    const size_t ns = (size_t)KCS_WT_NINT * N * T;
-    double *d_samples = nullptr;
-    if (cudaMalloc((void **)&d_samples, ns * sizeof(double)) != cudaSuccess ||
-        cudaMalloc((void **)&c->d_wcoef, ns * sizeof(float)) != cudaSuccess) {
-        cudaGetLastError();
-        if (d_samples) cudaFree(d_samples);
-        c->d_wcoef = nullptr;
-        c->err = "kcs_set_fit_precision: cudaMalloc failed";
-        return KCS_ERR_ALLOC;
-    }
-    c->ws_bytes += (long long)(ns * sizeof(float));
-    k_wtable_samples<<<(KCS_WT_NINT * N + 63) / 64, 64, sizeof(KFrame) * T, c->stream>>>(c->kin, d_samples);
-    c->launches++;
-    std::vector<double> smp(ns);
-    std::vector<float> coef(ns);
-    cudaError_t e = cudaMemcpyAsync(smp.data(), d_samples, ns * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-    cudaFree(d_samples);
-    if (e != cudaSuccess) { c->err = std::string("kcs_set_fit_precision: ") + cudaGetErrorString(e); return KCS_ERR_CUDA; }
-    // inverse of the Vandermonde matrix V[j][k] = s_j^k (the same for every interval and frame), long double Gauss-Jordan
-    long double V[N][2 * N];
-    const long double pi = 3.14159265358979323846264338327950288L;
-    for (int j = 0; j < N; ++j) {
-        const long double sj = cosl(pi * (2.0L * j + 1.0L) / (2.0L * N));
-        long double pw = 1.0L;
-        for (int k = 0; k < N; ++k) { V[j][k] = pw; pw *= sj; V[j][N + k] = (j == k) ? 1.0L : 0.0L; }
-    }
-    for (int col = 0; col < N; ++col) {
-        int piv = col;
-        for (int r = col + 1; r < N; ++r) if (fabsl(V[r][col]) > fabsl(V[piv][col])) piv = r;
-        for (int k = 0; k < 2 * N; ++k) { const long double t = V[col][k]; V[col][k] = V[piv][k]; V[piv][k] = t; }
-        const long double d = V[col][col];
-        for (int k = 0; k < 2 * N; ++k) V[col][k] /= d;
-        for (int r = 0; r < N; ++r) {
-            if (r == col) continue;
-            const long double f = V[r][col];
-            for (int k = 0; k < 2 * N; ++k) V[r][k] -= f * V[col][k];
-        }
-    }
-    for (int i = 0; i < KCS_WT_NINT; ++i)
-        for (int m = 0; m < T; ++m)
-            for (int k = 0; k < N; ++k) {
-                long double acc = 0.0L;
-                for (int j = 0; j < N; ++j) acc += V[k][N + j] * (long double)smp[((size_t)i * N + j) * T + m];
-                coef[((size_t)i * T + m) * N + k] = (float)acc;
-            }
-    e = cudaMemcpyAsync(c->d_wcoef, coef.data(), ns * sizeof(float), cudaMemcpyHostToDevice, c->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-    if (e != cudaSuccess) { c->err = std::string("kcs_set_fit_precision: ") + cudaGetErrorString(e); return KCS_ERR_CUDA; }
-    c->kin.wcoef = c->d_wcoef;
-    return KCS_OK;
-}
 
 int kcs_launch_ki_map(kcs_ctx *c, const float *theta, float *ki) {
     const long long nvox = (long long)c->n_vox;
@@ -565,17 +430,11 @@ int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const vo
     const double4 d4 = c->has_delta4 ? make_double4(c->delta4[0], c->delta4[1], c->delta4[2], c->delta4[3])
                                      : make_double4((double)delta, (double)delta, (double)delta, (double)delta);
     const bool opt = c->weighted || c->has_delta4 || c->nbr_mode != 6;
-    const bool f32 = c->fit_fp32 && !opt && c->kin.wcoef != nullptr;
-#define KCS_LM_GO2(TI, TO, OPT, F32)                                                                                   \
-    k_lm_step<TI, TO, OPT, F32><<<grid, KCS_LM_TPB, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, (const TI *)theta_in, (TO *)theta_out, \
+#define KCS_LM_GO2(TI, TO, OPT)                                                                                        \
+    k_lm_step<TI, TO, OPT><<<grid, KCS_LM_TPB, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, (const TI *)theta_in, (TO *)theta_out, \
                                                        (const TI *)lam_in, (TO *)lam_out, c->d_mask, c->d_vlist, c->n_inmask2, nvox, (double)gamma,  \
                                                        d4, c->nbr_mode, cost, c->lm_state, nfit)
-#define KCS_LM_GO(TI, TO)                                                                                              \
-    do {                                                                                                               \
-        if (opt) KCS_LM_GO2(TI, TO, true, false);                                                                      \
-        else if (f32) KCS_LM_GO2(TI, TO, false, true);                                                                 \
-        else KCS_LM_GO2(TI, TO, false, false);                                                                         \
-    } while (0)
+#define KCS_LM_GO(TI, TO) do { if (opt) KCS_LM_GO2(TI, TO, true); else KCS_LM_GO2(TI, TO, false); } while (0)
     if (!in_f64 && !out_f64) KCS_LM_GO(float, float);
     else if (!in_f64 && out_f64) KCS_LM_GO(float, double);
     else if (in_f64 && out_f64) KCS_LM_GO(double, double);
