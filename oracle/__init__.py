@@ -274,13 +274,17 @@ class Oracle:
         return np.concatenate(xs, axis=1), np.concatenate(ths, axis=1), np.concatenate(lams, axis=0)
 
     @staticmethod
-    def set_lm_options(frame_w=None, neighbourhood=6, delta4=None):
-        """S8(f)2 / S8(f)4: weighted least squares, the 3x3-clique neighbourhood (10), per-parameter Huber thresholds.
-        Oracle-wide; call with no arguments to restore the defaults."""
+    def set_lm_options(frame_w=None, neighbourhood=6, delta4=None, prior_curvature=False, box_lo=None, box_hi=None):
+        """S8(f)2 / S8(f)4: weighted least squares, the 3x3-clique neighbourhood (10), per-parameter Huber thresholds, Huber
+        curvature in the LM matrix, another parameter box (lo == hi fixes a parameter).  Oracle-wide; call with no
+        arguments to restore the defaults."""
         fw = None if frame_w is None else _f64(frame_w)
         d4 = None if delta4 is None else _f64(delta4)
+        lo = None if box_lo is None else _f64(box_lo)
+        hi = None if box_hi is None else _f64(box_hi)
         _L().kcso_set_lm_options(None if fw is None else _p(fw), C.c_int(0 if fw is None else fw.size), C.c_int(neighbourhood),
                                  None if d4 is None else _p(d4))
+        _L().kcso_set_lm_options2(C.c_int(1 if prior_curvature else 0), None if lo is None else _p(lo), None if hi is None else _p(hi))
 
     @staticmethod
     def ki_map(theta):

@@ -492,8 +492,22 @@ void kcso_set_lm_options(const double *frame_w, int n_frames, int neighbourhood,
 static double frame_w(int m) { return lm_has_w ? lm_w[m] : 1.0; }
 static double delta_of(int p, double delta) { return lm_has_delta4 ? lm_delta4[p] : delta; }
 
-static const double BOX_LO[4] = {0.0, 1e-4, 0.0, 0.0};
-static const double BOX_HI[4] = {2.0, 2.0, 1.0, 1.0};
+static const double BOX_LO_Q16[4] = {0.0, 1e-4, 0.0, 0.0};
+static const double BOX_HI_Q16[4] = {2.0, 2.0, 1.0, 1.0};
+/* S8(f)2 / S8(f)4, second part (kcso_set_lm_options2; defaults = Q16 box, no curvature):
+ *   box: other bounds per parameter; lo_p == hi_p FIXES parameter p (its Jacobian column is zero and it sits at lo_p):
+ *     k3 = 0 is the one-tissue compartment model, fixed vB a fit without a blood-volume term;
+ *   prior curvature: the Gauss-Newton curvature of the Huber sum, gamma sum_k H''(xi_p - xi_k,p) with H'' = 1 inside the
+ *     threshold and 0 outside, is added to the diagonal of the LM matrix (eq. 4 as printed has only lambda I). */
+static double BOX_LO[4] = {0.0, 1e-4, 0.0, 0.0}, BOX_HI[4] = {2.0, 2.0, 1.0, 1.0};
+static int lm_curv = 0;
+void kcso_set_lm_options2(int prior_curvature, const double *box_lo, const double *box_hi) {
+    lm_curv = prior_curvature != 0;
+    for (int p = 0; p < 4; ++p) {
+        BOX_LO[p] = box_lo ? box_lo[p] : BOX_LO_Q16[p];
+        BOX_HI[p] = box_hi ? box_hi[p] : BOX_HI_Q16[p];
+    }
+}
 
 static double objective(const kcso_config *c, const double *xv, const double xi[4], const double *Fv,
                         const double *nbr, int n_nbr, double gamma, double delta) {
@@ -548,7 +562,12 @@ static double lm_step_voxel(const kcso_config *c, const double *tab, const doubl
                             const double *nbr, int n_nbr, double gamma, double delta,
                             double *Fv, double *Jv, double *Ft) {
     const int T = c->n_frames;
+    for (int p = 0; p < 4; ++p)
+        if (BOX_LO[p] == BOX_HI[p]) xi[p] = BOX_LO[p];   /* a fixed parameter sits at its value */
     tac_voxel(c, tab, xi, Fv, Jv);
+    for (int p = 0; p < 4; ++p)
+        if (BOX_LO[p] == BOX_HI[p])
+            for (int m = 0; m < T; ++m) Jv[p * T + m] = 0.0; /* ... and is not fitted */
     const double phi_old = objective(c, xv, xi, Fv, nbr, n_nbr, gamma, delta);
     double JtJ[4][4] = {{0}}, g[4] = {0};
     for (int p = 0; p < 4; ++p) {
@@ -566,6 +585,10 @@ static double lm_step_voxel(const kcso_config *c, const double *tab, const doubl
     double M[4][4], d[4];
     for (int p = 0; p < 4; ++p)
         for (int q = 0; q < 4; ++q) M[p][q] = JtJ[p][q] + (p == q ? *lam : 0.0);
+    if (lm_curv)
+        for (int p = 0; p < 4; ++p)
+            for (int q = 0; q < n_nbr; ++q)
+                if (fabs(xi[p] - nbr[q * 4 + p]) <= delta_of(p, delta)) M[p][p] += gamma;
     if (!chol4_solve(M, g, d)) { /* not positive definite: treated as a rejected step */
         *lam = fmin(10.0 * *lam, 1e30);
         return phi_old;

@@ -87,6 +87,10 @@ void kcso_map_lm(const kcso_config *c, const double *x, double *theta, double *l
  * of P:114 plus +-z); delta4[4] one Huber threshold per parameter map (the scalar delta argument is then ignored). */
 void kcso_set_lm_options(const double *frame_w, int n_frames, int neighbourhood, const double *delta4);
 
+/* second part: prior_curvature != 0 adds gamma sum_k H''(xi_p - xi_k,p) to the diagonal of the LM matrix; box_lo / box_hi
+ * (NULL = Q16) replace the parameter box, lo_p == hi_p fixes parameter p (one-tissue model: k3 in [0, 0]). */
+void kcso_set_lm_options2(int prior_curvature, const double *box_lo, const double *box_hi);
+
 /* Q15a knob (oracle only): relative slack of the LM acceptance test, default 1e-6. */
 void kcso_set_lm_accept_slack(double s);
 double kcso_get_lm_accept_slack(void);

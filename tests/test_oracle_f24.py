@@ -107,3 +107,48 @@ def test_zero_weight_drops_the_frame():
     th_s, lam_s, c_s = o2.map_lm(x[:-2], start, lam0, 0.0, 0.01, 5, want_cost=True)
     np.testing.assert_allclose(th_w, th_s, rtol=1e-12, atol=1e-15)
     np.testing.assert_allclose(c_w, c_s, rtol=1e-12)
+
+
+def test_curvature_with_no_data_is_one_newton_step_to_the_neighbour_mean():
+    """All frame weights 0: Phi = gamma sum_p sum_k H(xi_p - xi_k,p), a quadratic while every difference is inside delta.
+    With the Huber curvature in the LM matrix, lambda_0 = 1e-3 max diag J^T W J = 0 and M = gamma n_k I, so one step lands
+    every voxel EXACTLY on the mean of its neighbours in the previous iterate -- a different code path from the
+    gradient, checked here against numpy means.  (Without the curvature the matrix is zero and the step is rejected.)"""
+    cfg, o, mask, x, start = _problem(nx=5, ny=4, nz=3)
+    T = cfg["n_frames"]
+    rng = np.random.default_rng(5)
+    prev = np.array(ki.GREY)[:, None, None, None] * (1 + 0.01 * rng.uniform(-1, 1, size=(4, 3, 4, 5)))
+    lam0 = np.zeros((3, 4, 5))
+    Oracle.set_lm_options(frame_w=np.zeros(T), neighbourhood=10, delta4=[1.0] * 4, prior_curvature=True)
+    new, lam, cost = o.map_lm(x, prev, lam0, 2.5, 0.0, 1, want_cost=True)
+    offs = [(0, 0, -1), (0, 0, 1), (0, -1, 0), (0, 1, 0), (-1, 0, 0), (1, 0, 0), (0, -1, -1), (0, -1, 1), (0, 1, -1), (0, 1, 1)]
+    for z in range(3):
+        for j in range(4):
+            for i in range(5):
+                nb = [prev[:, z + dz, j + dj, i + di] for dz, dj, di in offs
+                      if 0 <= z + dz < 3 and 0 <= j + dj < 4 and 0 <= i + di < 5]
+                np.testing.assert_allclose(new[:, z, j, i], np.mean(nb, axis=0), rtol=1e-13)
+    Oracle.set_lm_options(frame_w=np.zeros(T), neighbourhood=10, delta4=[1.0] * 4, prior_curvature=False)
+    stuck = o.map_lm(x, prev, lam0, 2.5, 0.0, 1)[0]
+    assert np.array_equal(stuck, prev)
+
+
+def test_fixed_parameter_gives_the_one_tissue_model():
+    """box k3 in [0, 0]: the fit of the one-tissue compartment model.  Noise-free one-tissue curves are recovered to 1e-6
+    from a +-30 % start, k3 stays exactly 0 and takes no part in the solve; the default box is untouched by a reset."""
+    cfg, o, mask, x, start = _problem(nx=4, ny=4, nz=1)
+    rng = np.random.default_rng(9)
+    th_true = np.array([0.08, 0.12, 0.0, 0.04])[:, None, None, None] * (1 + 0.2 * rng.uniform(-1, 1, size=(4, 1, 4, 4)))
+    th_true[2] = 0.0
+    x = o.kinetic_eval(th_true)
+    start = th_true * (1 + 0.3 * rng.uniform(-1, 1, size=th_true.shape))
+    start[2] = 0.05                                   # a wrong k3 in the start: the fixed value must replace it
+    Oracle.set_lm_options(box_lo=[0.0, 1e-4, 0.0, 0.0], box_hi=[2.0, 2.0, 0.0, 1.0])
+    th, lam = o.map_lm(x, start, np.zeros((1, 4, 4)), 0.0, 0.01, 60)
+    assert np.all(th[2] == 0.0)
+    np.testing.assert_allclose(th[[0, 1, 3]], th_true[[0, 1, 3]], rtol=1e-6)
+    Oracle.set_lm_options()
+    th2 = th_true.copy()
+    th2[2] = 0.05
+    free = o.map_lm(o.kinetic_eval(th2), start, np.zeros((1, 4, 4)), 0.0, 0.01, 60)[0]
+    np.testing.assert_allclose(free[2], 0.05, rtol=1e-5)   # default box again: k3 is fitted
