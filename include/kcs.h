@@ -144,14 +144,20 @@ int kcs_map_lm(kcs_ctx *ctx, const float *x, float *theta, float *lambda, float 
                int n_steps, float *cost);
 
 /* Options of the fit beyond the hot path, for the kcs_map_lm / kcs_icm_* calls that follow; all
- * pointers [host]; SYNCHRONISES the stream.  NULL / 6 / NULL restore the defaults.
- *   frame_weights[T] >= 0   weighted least squares: data term 1/2 sum_m w_m (x_m - F_m)^2 (e.g. frame-duration or
- *                           inverse-variance weights); w_m = 0 drops frame m from the fit
- *   neighbourhood           6: +-x, +-y, +-z (Q13).  10: the 8 in-plane neighbours of the paper's 3x3 clique (P:114,
- *                           Fig. 1 caption P:47) plus +-z; unit weights, in-volume and in-mask neighbours only
- *   delta4[4]               one Huber threshold per parameter map (K1, k2, k3, vB); the scalar delta argument of the
- *                           calls is then ignored */
-int kcs_set_fit_options(kcs_ctx *ctx, const double *frame_weights, int neighbourhood, const double *delta4);
+ * pointers [host]; SYNCHRONISES the stream.  opt == NULL restores the defaults (NULL, 6, NULL, 0, NULL, NULL). */
+typedef struct {
+    const double *frame_weights; /* [T] >= 0: weighted least squares, data term 1/2 sum_m w_m (x_m - F_m)^2 (e.g. frame-duration
+                                  * or inverse-variance weights); w_m = 0 drops frame m from the fit */
+    int neighbourhood;           /* 6: +-x, +-y, +-z (Q13).  10: the 8 in-plane neighbours of the paper's 3x3 clique (P:114,
+                                  * Fig. 1 caption P:47) plus +-z; unit weights, in-volume and in-mask neighbours only */
+    const double *delta4;        /* [4] one Huber threshold per parameter map (K1, k2, k3, vB); the scalar delta argument of
+                                  * the calls is then ignored */
+    int prior_curvature;         /* != 0: the Gauss-Newton curvature of the Huber sum, gamma sum_k H''(xi_p - xi_k,p), joins
+                                  * lambda on the diagonal of the LM matrix (eq. 4 as printed has lambda I only) */
+    const double *box_lo;        /* [4], [4]: another parameter box than Q16's (both or neither).  lo_p == hi_p FIXES parameter */
+    const double *box_hi;        /* p: it sits at lo_p and is not fitted -- k3 in [0, 0] is the one-tissue compartment model */
+} kcs_fit_options;
+int kcs_set_fit_options(kcs_ctx *ctx, const kcs_fit_options *opt);
 
 /* the macro-parameter map K_i = K1 k3 / (k2 + k3) (net influx rate; 0 where k2 + k3 = 0) from
  * theta[4][nz][ny][nx]; ki[nz][ny][nx] (device).  Evaluated for every voxel. */

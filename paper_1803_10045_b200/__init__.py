@@ -56,6 +56,11 @@ class _Config(C.Structure):
     ]
 
 
+class _FitOptions(C.Structure):
+    _fields_ = [("frame_weights", C.POINTER(C.c_double)), ("neighbourhood", C.c_int), ("delta4", C.POINTER(C.c_double)),
+                ("prior_curvature", C.c_int), ("box_lo", C.POINTER(C.c_double)), ("box_hi", C.POINTER(C.c_double))]
+
+
 _lib = None
 
 
@@ -97,7 +102,7 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.kcs_kinetic_eval.argtypes = [vp, fp, fp, fp]
     lib.kcs_ki_map.argtypes = [vp, fp, fp]
     lib.kcs_set_multiplicative.argtypes = [vp, fp]
-    lib.kcs_set_fit_options.argtypes = [vp, vp, i, vp]
+    lib.kcs_set_fit_options.argtypes = [vp, vp]
     lib.kcs_map_lm.argtypes = [vp, fp, fp, fp, f, f, i, fp]
     lib.kcs_icm_iteration.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, i]
     lib.kcs_icm_run.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, f, i, i]
@@ -255,14 +260,17 @@ class Context:
         """mult: float32 CUDA tensor [nz][A][B] (attenuation x normalisation factors) or None for unit factors."""
         self._check(self._lib.kcs_set_multiplicative(self._h, None if mult is None else _dev(mult, (self.nz, self.A, self.B))))
 
-    def set_fit_options(self, frame_weights=None, neighbourhood: int = 6, delta4=None):
-        """Weighted least squares, the 3x3-clique neighbourhood (10), per-parameter Huber thresholds; no arguments = defaults."""
-        fw = None if frame_weights is None else np.ascontiguousarray(frame_weights, dtype=np.float64)
-        d4 = None if delta4 is None else np.ascontiguousarray(delta4, dtype=np.float64)
+    def set_fit_options(self, frame_weights=None, neighbourhood: int = 6, delta4=None, prior_curvature: bool = False,
+                        box_lo=None, box_hi=None):
+        """kcs_fit_options: weighted least squares, the 3x3-clique neighbourhood (10), per-parameter Huber thresholds, Huber
+        curvature in the LM matrix, another parameter box (lo == hi fixes a parameter); no arguments = defaults."""
+        arr = lambda a, n: None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+        fw, d4, lo, hi = arr(frame_weights, self.T), arr(delta4, 4), arr(box_lo, 4), arr(box_hi, 4)
         assert fw is None or fw.size == self.T
-        assert d4 is None or d4.size == 4
-        self._check(self._lib.kcs_set_fit_options(self._h, None if fw is None else fw.ctypes.data_as(C.c_void_p), neighbourhood,
-                                                  None if d4 is None else d4.ctypes.data_as(C.c_void_p)))
+        assert all(a is None or a.size == 4 for a in (d4, lo, hi))
+        ptr = lambda a: None if a is None else a.ctypes.data_as(C.POINTER(C.c_double))
+        o = _FitOptions(ptr(fw), neighbourhood, ptr(d4), int(bool(prior_curvature)), ptr(lo), ptr(hi))
+        self._check(self._lib.kcs_set_fit_options(self._h, C.byref(o)))
 
     def ki_map(self, theta, ki):
         shp = (self.nz, self.ny, self.nx)

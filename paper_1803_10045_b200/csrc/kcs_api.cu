@@ -354,6 +354,9 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->nbr_mode = 6;
     c->has_delta4 = false;
     c->weighted = false;
+    c->prior_curv = c->custom_box = false;
+    { const double lo[4] = {0.0, 1e-4, 0.0, 0.0}, hi[4] = {2.0, 2.0, 1.0, 1.0};  // Q16
+      for (int p = 0; p < 4; ++p) { c->box_lo[p] = lo[p]; c->box_hi[p] = hi[p]; } }
 
     std::vector<int> vlist;
     for (int q = 0; q < nx * ny; ++q)
@@ -532,25 +535,37 @@ static int lm_steps(kcs_ctx *c, const float *x, int x_inner, int Tp, float *thet
     return KCS_OK;
 }
 
-int kcs_set_fit_options(kcs_ctx *c, const double *frame_weights, int neighbourhood, const double *delta4) {
+int kcs_set_fit_options(kcs_ctx *c, const kcs_fit_options *opt) {
     if (!c) return KCS_ERR_NULL;
-    if (neighbourhood != 6 && neighbourhood != 10) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: neighbourhood must be 6 or 10");
+    static const kcs_fit_options defaults = {nullptr, 6, nullptr, 0, nullptr, nullptr};
+    if (!opt) opt = &defaults;
+    if (opt->neighbourhood != 6 && opt->neighbourhood != 10) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: neighbourhood must be 6 or 10");
     const int T = c->cfg.n_frames;
     for (int m = 0; m < T; ++m)
-        if (frame_weights && !(frame_weights[m] >= 0.0)) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: negative frame weight");
+        if (opt->frame_weights && !(opt->frame_weights[m] >= 0.0)) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: negative frame weight");
     for (int p = 0; p < 4; ++p)
-        if (delta4 && !(delta4[p] >= 0.0)) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: negative delta");
+        if (opt->delta4 && !(opt->delta4[p] >= 0.0)) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: negative delta");
+    if ((opt->box_lo == nullptr) != (opt->box_hi == nullptr)) return fail(c, KCS_ERR_NULL, "kcs_set_fit_options: box_lo and box_hi go together");
+    for (int p = 0; p < 4; ++p)
+        if (opt->box_lo && !(opt->box_lo[p] <= opt->box_hi[p])) return fail(c, KCS_ERR_SHAPE, "kcs_set_fit_options: box_lo > box_hi");
     c->opt_gen++;
     c->weighted = false;
     for (int m = 0; m < T; ++m) {
-        c->h_frames[m].w = frame_weights ? frame_weights[m] : 1.0;
+        c->h_frames[m].w = opt->frame_weights ? opt->frame_weights[m] : 1.0;
         if (c->h_frames[m].w != 1.0) c->weighted = true;
     }
     KCS_CUDA_OK(c, cudaStreamSynchronize(c->stream));  // kernels in flight still read the old table
     KCS_CUDA_OK(c, cudaMemcpy(c->d_frames, c->h_frames.data(), sizeof(KFrame) * T, cudaMemcpyHostToDevice));
-    c->nbr_mode = neighbourhood;
-    c->has_delta4 = delta4 != nullptr;
-    for (int p = 0; p < 4; ++p) c->delta4[p] = delta4 ? delta4[p] : 0.0;
+    c->nbr_mode = opt->neighbourhood;
+    c->has_delta4 = opt->delta4 != nullptr;
+    for (int p = 0; p < 4; ++p) c->delta4[p] = opt->delta4 ? opt->delta4[p] : 0.0;
+    c->prior_curv = opt->prior_curvature != 0;
+    c->custom_box = opt->box_lo != nullptr;
+    const double lo[4] = {0.0, 1e-4, 0.0, 0.0}, hi[4] = {2.0, 2.0, 1.0, 1.0};  // Q16
+    for (int p = 0; p < 4; ++p) {
+        c->box_lo[p] = opt->box_lo ? opt->box_lo[p] : lo[p];
+        c->box_hi[p] = opt->box_hi ? opt->box_hi[p] : hi[p];
+    }
     return KCS_OK;
 }
 

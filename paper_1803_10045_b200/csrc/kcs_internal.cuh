@@ -98,6 +98,8 @@ struct kcs_ctx {
     bool weighted;                    // some frame weight differs from 1 (S8(f)4)
     bool has_delta4;                  // one Huber threshold per parameter map instead of the scalar argument
     double delta4[4];
+    bool prior_curv, custom_box;      // Huber curvature in the LM matrix; a parameter box other than Q16's
+    double box_lo[4], box_hi[4];
     unsigned char *d_mask;            // [ny][nx]
     int *d_vlist;                     // in-mask pixel indices j*nx+i of one slice, ascending
     int n_inmask2;                    // their count

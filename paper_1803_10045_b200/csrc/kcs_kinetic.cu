@@ -29,6 +29,15 @@
 
 namespace {
 
+// Options of the fit handed to k_lm_step by value (kcs_set_fit_options; the default kernel reads delta[0] only).
+struct LmOpt {
+    double delta[4];      // Huber threshold per parameter map
+    double lo[4], hi[4];  // parameter box; lo == hi fixes a parameter
+    int nq;               // neighbours: 6 or 10
+    int curv;             // Huber curvature in the LM matrix
+    int fixmask;          // bit p: parameter p is fixed
+};
+
 // E1(a; t) = int_0^t u e^{-a u} du, given z = a t and em1 = expm1(-z).
 __device__ __forceinline__ double E1_of(double a, double t, double z, double em1) {
     if (z < 0.5) {
@@ -247,12 +256,15 @@ __device__ __forceinline__ bool chol4(const double m[10], const double g[4], dou
 
 // Data part of the normal equations at theta: out[0..9] = J^T J (packed lower triangle), out[10..13] = J^T r,
 // out[14] = 1/2 sum r^2.  One (not inlined) copy of the model code serves both evaluations of a step.
+// WLS (the OPT kernel): frame weights, and `fixmask` bit p set = parameter p is fixed (its Jacobian column is zero).
 template <bool WLS>
 __device__ __forceinline__ void lm_eval(KKin kin, const KFrame *fr, const float *__restrict__ x, size_t xbase, size_t xstride,
-                                     double K1, double k2, double k3, double vB, double *out) {
+                                     double K1, double k2, double k3, double vB, int fixmask, double *out) {
     double JtJ[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, gr[4] = {0, 0, 0, 0}, phi = 0.0;
+    const double f0 = (fixmask & 1) ? 0.0 : 1.0, f1 = (fixmask & 2) ? 0.0 : 1.0, f2 = (fixmask & 4) ? 0.0 : 1.0, f3 = (fixmask & 8) ? 0.0 : 1.0;
     tac_stream<true>(kin, fr, K1, k2, k3, vB, [&](int m, double Fm, double j0, double j1, double j2, double j3) {
         const double r = (double)x[xbase + m * xstride] - Fm;
+        if (WLS) { j0 *= f0; j1 *= f1; j2 *= f2; j3 *= f3; }
         // S8(f)4: frame weights w_m (WLS; compiled out of the default path) -- J^T W J, J^T W r, 1/2 r^T W r
         const double w = WLS ? fr[m].w : 1.0;
         const double w0 = WLS ? w * j0 : j0, w1 = WLS ? w * j1 : j1, w2 = WLS ? w * j2 : j2, w3 = WLS ? w * j3 : j3;
@@ -284,7 +296,7 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
                                                  const TI *__restrict__ th_in, TO *__restrict__ th_out,
                                                  const TI *lam_in, TO *lam_out,  // may alias: each thread touches its own element
                                                  const unsigned char *__restrict__ mask, const int *__restrict__ vlist, int M2,
-                                                 long long nvox, double gamma, double4 delta4, int nq, float *cost,
+                                                 long long nvox, double gamma, LmOpt o, float *cost,
                                                  double *__restrict__ st, long long nfit) {
     constexpr int NQ = OPT ? 10 : 6;
     constexpr bool WLS = OPT;
@@ -305,10 +317,14 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
 
     double xi[4];
 #pragma unroll
-    for (int p = 0; p < 4; ++p) xi[p] = th_in[(size_t)p * nvox + v];
+    for (int p = 0; p < 4; ++p) {
+        xi[p] = th_in[(size_t)p * nvox + v];
+        if (OPT && ((o.fixmask >> p) & 1)) xi[p] = o.lo[p];  // a fixed parameter sits at its value
+    }
     // Q13: in-volume, in-mask 6-neighbourhood of the previous iterate (Jacobi); NQ = 10 (S8(f)2): the four in-plane
     // diagonals of the 3x3 clique as well
-    const double delta[4] = {delta4.x, OPT ? delta4.y : delta4.x, OPT ? delta4.z : delta4.x, OPT ? delta4.w : delta4.x};
+    const double delta[4] = {o.delta[0], OPT ? o.delta[1] : o.delta[0], OPT ? o.delta[2] : o.delta[0], OPT ? o.delta[3] : o.delta[0]};
+    const int nq = o.nq;
     double nb[NQ][4];
     int nn = 0;
     {
@@ -333,7 +349,7 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
 
     double ev[15];
     if (FIRST) {
-        lm_eval<WLS>(kin, fr, x, xa.base, xa.fstride, xi[0], xi[1], xi[2], xi[3], ev);
+        lm_eval<WLS>(kin, fr, x, xa.base, xa.fstride, xi[0], xi[1], xi[2], xi[3], o.fixmask, ev);
         if (!LAST) {
 #pragma unroll
             for (int q = 0; q < 15; ++q) st[(size_t)q * nfit + t] = ev[q];  // kept if this step is rejected
@@ -343,12 +359,14 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
         for (int q = 0; q < 15; ++q) ev[q] = st[(size_t)q * nfit + t];
     }
     double gr[4] = {ev[10], ev[11], ev[12], ev[13]}, phi_old = ev[14];
+    double curv[4] = {0.0, 0.0, 0.0, 0.0};  // OPT: Gauss-Newton curvature of the Huber sum, gamma sum_k H''
     for (int q = 0; q < nn; ++q)
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
             const double tt = xi[p] - nb[q][p];
             phi_old += gamma * huber(tt, delta[p]);
             gr[p] -= gamma * huber_d(tt, delta[p]);
+            if (OPT && o.curv && fabs(tt) <= delta[p]) curv[p] += gamma;
         }
 
     double lam = lam_in[v];
@@ -357,6 +375,7 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
 #pragma unroll
     for (int q = 0; q < 10; ++q) M[q] = ev[q];
     M[0] += lam; M[2] += lam; M[5] += lam; M[9] += lam;
+    if (OPT) { M[0] += curv[0]; M[2] += curv[1]; M[5] += curv[2]; M[9] += curv[3]; }
     double d[4];
     double phi = phi_old;
     if (!chol4(M, gr, d)) {
@@ -365,8 +384,8 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
         const double lo[4] = {0.0, 1e-4, 0.0, 0.0}, hi[4] = {2.0, 2.0, 1.0, 1.0};  // Q16
         double xt[4];
 #pragma unroll
-        for (int p = 0; p < 4; ++p) xt[p] = fmin(fmax(xi[p] + d[p], lo[p]), hi[p]);
-        lm_eval<WLS>(kin, fr, x, xa.base, xa.fstride, xt[0], xt[1], xt[2], xt[3], ev);
+        for (int p = 0; p < 4; ++p) xt[p] = fmin(fmax(xi[p] + d[p], OPT ? o.lo[p] : lo[p]), OPT ? o.hi[p] : hi[p]);
+        lm_eval<WLS>(kin, fr, x, xa.base, xa.fstride, xt[0], xt[1], xt[2], xt[3], o.fixmask, ev);
         double phi_new = ev[14];
         for (int q = 0; q < nn; ++q)
 #pragma unroll
@@ -427,13 +446,21 @@ int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const vo
     if (nfit == 0) return KCS_OK;
     const unsigned grid = (unsigned)((nfit + KCS_LM_TPB - 1) / KCS_LM_TPB);
     ProfScope ps(c, KCS_K_LM);
-    const double4 d4 = c->has_delta4 ? make_double4(c->delta4[0], c->delta4[1], c->delta4[2], c->delta4[3])
-                                     : make_double4((double)delta, (double)delta, (double)delta, (double)delta);
-    const bool opt = c->weighted || c->has_delta4 || c->nbr_mode != 6;
+    LmOpt o;
+    o.fixmask = 0;
+    for (int p = 0; p < 4; ++p) {
+        o.delta[p] = c->has_delta4 ? c->delta4[p] : (double)delta;
+        o.lo[p] = c->box_lo[p];
+        o.hi[p] = c->box_hi[p];
+        if (o.lo[p] == o.hi[p]) o.fixmask |= 1 << p;
+    }
+    o.nq = c->nbr_mode;
+    o.curv = c->prior_curv ? 1 : 0;
+    const bool opt = c->weighted || c->has_delta4 || c->nbr_mode != 6 || c->prior_curv || c->custom_box;
 #define KCS_LM_GO2(TI, TO, OPT)                                                                                        \
     k_lm_step<TI, TO, OPT><<<grid, KCS_LM_TPB, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, (const TI *)theta_in, (TO *)theta_out, \
                                                        (const TI *)lam_in, (TO *)lam_out, c->d_mask, c->d_vlist, c->n_inmask2, nvox, (double)gamma,  \
-                                                       d4, c->nbr_mode, cost, c->lm_state, nfit)
+                                                       o, cost, c->lm_state, nfit)
 #define KCS_LM_GO(TI, TO) do { if (opt) KCS_LM_GO2(TI, TO, true); else KCS_LM_GO2(TI, TO, false); } while (0)
     if (!in_f64 && !out_f64) KCS_LM_GO(float, float);
     else if (!in_f64 && out_f64) KCS_LM_GO(float, double);

@@ -53,6 +53,10 @@ def _frac(thg, tho, mask):
     dict(neighbourhood=10),                                                      # the 3x3 clique alone
     dict(delta4=[0.004, 0.02, 0.007, 0.011]),                                    # per-parameter thresholds alone
     dict(frame_weights="ramp", neighbourhood=10, delta4=[0.004, 0.02, 0.007, 0.011]),
+    dict(prior_curvature=True),                                                  # Huber curvature in the LM matrix
+    dict(box_lo=[0.0, 1e-4, 0.0, 0.0], box_hi=[2.0, 2.0, 0.0, 1.0]),             # k3 fixed at 0: the one-tissue model
+    dict(neighbourhood=10, delta4=[0.004, 0.02, 0.007, 0.011], prior_curvature=True,
+         box_lo=[0.01, 0.02, 0.0, 0.03], box_hi=[0.5, 1.0, 0.2, 0.03]),          # a tighter box, vB fixed at 0.03
 ])
 def test_map_lm_with_fit_options(opts):
     cfg = ki.small_config(nx=45, ny=37, nz=3, n_angles=30, n_bins=51, n_subsets=5, n_steps=57, sched="C3")
@@ -68,7 +72,8 @@ def test_map_lm_with_fit_options(opts):
     lam0 = np.zeros(x.shape[1:])
     plain_th, plain_lam = dev(start), dev(lam0)
     ctx.map_lm(dev(x), plain_th, plain_lam, 3e5, 0.01, 3)
-    Oracle.set_lm_options(frame_w=opts.get("frame_weights"), neighbourhood=opts.get("neighbourhood", 6), delta4=opts.get("delta4"))
+    Oracle.set_lm_options(frame_w=opts.get("frame_weights"), neighbourhood=opts.get("neighbourhood", 6), delta4=opts.get("delta4"),
+                          prior_curvature=opts.get("prior_curvature", False), box_lo=opts.get("box_lo"), box_hi=opts.get("box_hi"))
     ctx.set_fit_options(**opts)
     for gamma in (0.0, 3e5):
         for n_steps in (1, 4):
@@ -80,7 +85,11 @@ def test_map_lm_with_fit_options(opts):
             m = mask > 0
             assert np.mean(np.abs(host(cost)[:, m] - costo[:, m]) <= 1e-3 * np.abs(costo[:, m]) + 1e-6) >= 0.999
             assert np.mean(np.abs(host(lam)[:, m] - lamo[:, m]) <= 1e-3 * np.abs(lamo[:, m])) >= 0.999
-    if "neighbourhood" in opts or "delta4" in opts:          # the options matter at gamma = 3e5
+    if "box_lo" in opts:                                     # fixed parameters sit exactly at their value
+        for p in range(4):
+            if opts["box_lo"][p] == opts["box_hi"][p]:
+                assert np.all(host(th)[p][:, mask > 0] == np.float32(opts["box_lo"][p]))
+    if "neighbourhood" in opts or "delta4" in opts or "prior_curvature" in opts:   # the options matter at gamma = 3e5
         assert not torch.equal(th, plain_th)
     ctx.set_fit_options()                                    # defaults: bit for bit the plain fit again
     th, lam = dev(start), dev(lam0)
@@ -112,6 +121,31 @@ def test_icm_iteration_with_fit_options():
     ctx.close()
 
 
+def test_curvature_alone_is_one_newton_step_to_the_neighbour_mean():
+    """The oracle's pin on the GPU: all frame weights 0, every difference inside delta, Huber curvature on -- one step puts
+    every voxel on the mean of its (10) neighbours of the previous iterate, to fp32 rounding of the stored maps."""
+    cfg = ki.small_config(nx=20, ny=18, nz=3, n_angles=8, n_bins=20, n_subsets=2)
+    kcs = _kcs()
+    ctx = kcs.Context(cfg, mask=np.ones((18, 20), dtype=np.uint8))
+    T = cfg["n_frames"]
+    rng = np.random.default_rng(5)
+    prev = np.float32(np.array(ki.GREY)[:, None, None, None] * (1 + 0.01 * rng.uniform(-1, 1, size=(4, 3, 18, 20)))).astype(np.float64)
+    ctx.set_fit_options(frame_weights=np.zeros(T), neighbourhood=10, delta4=[1.0] * 4, prior_curvature=True)
+    th, lam = dev(prev), dev(np.zeros((3, 18, 20)))
+    x = torch.ones((T, 3, 18, 20), dtype=torch.float32, device="cuda")
+    ctx.map_lm(x, th, lam, 2.5, 0.0, 1)
+    want = np.zeros_like(prev)
+    cnt = np.zeros((3, 18, 20))
+    for dz, dj, di in [(0, 0, -1), (0, 0, 1), (0, -1, 0), (0, 1, 0), (-1, 0, 0), (1, 0, 0), (0, -1, -1), (0, -1, 1), (0, 1, -1), (0, 1, 1)]:
+        src = (slice(max(dz, 0), 3 + min(dz, 0)), slice(max(dj, 0), 18 + min(dj, 0)), slice(max(di, 0), 20 + min(di, 0)))
+        dst = (slice(max(-dz, 0), 3 + min(-dz, 0)), slice(max(-dj, 0), 18 + min(-dj, 0)), slice(max(-di, 0), 20 + min(-di, 0)))
+        want[(slice(None),) + dst] += prev[(slice(None),) + src]
+        cnt[dst] += 1
+    want /= cnt[None]
+    np.testing.assert_allclose(host(th), want, rtol=2e-7)
+    ctx.close()
+
+
 def test_fit_option_errors():
     kcs = _kcs()
     cfg = ki.small_config()
@@ -121,5 +155,8 @@ def test_fit_option_errors():
     assert e.value.code == -2
     with pytest.raises(kcs.KcsError) as e:
         ctx.set_fit_options(frame_weights=-np.ones(cfg["n_frames"]))
+    assert e.value.code == -2
+    with pytest.raises(kcs.KcsError) as e:
+        ctx.set_fit_options(box_lo=[0.0, 0.5, 0.0, 0.0], box_hi=[1.0, 0.1, 1.0, 1.0])
     assert e.value.code == -2
     ctx.close()
