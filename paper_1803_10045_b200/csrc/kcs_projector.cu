@@ -435,11 +435,14 @@ int kcs_launch_build_wtab(kcs_ctx *c) {
 // voxels: 1.25 L1 wavefronts per voxel-angle instead of 3.  Weights come from the k_build_wtab table (L2 resident:
 // it is the same for every slice and frame).  No atomics: run-to-run deterministic.
 // Two instantiations are used (round 2, C4, per subset launch; results are bit-identical):
-//   <2, true>   two slices per thread, the record of angle l+1 requested before the math of angle l, 4 CTAs per SM: the
+//   <2, true, .>   two slices per thread, the record of angle l+1 requested before the math of angle l, 4 CTAs per SM: the
 //               plain back-projection (all 252 angles: 47.7 ms against 54.3);
-//   <1, false>  one slice per thread, no prefetch, 80 registers, 6 CTAs per SM: the fused OSL update, whose epilogue
+//   <1, false, .>  one slice per thread, no prefetch, 80 registers, 6 CTAs per SM: the fused OSL update, whose epilogue
 //               (x and F from HBM) overlaps other CTAs' angle loops better at 24 warps per SM (2.50 ms against 2.64).
-template <int ZB, bool PIPE>
+// TPC: the padded frame count as a compile-time constant (32 on the ICM path of C2-C4: the window loads then take immediate
+// offsets) or 0 for "read p.Tp".  Record and row pointers advance by constant strides from angle to angle; the loop body of
+// <1, false, 32> went from 150 to SASS instructions per angle for 80 FFMA with both.
+template <int ZB, bool PIPE, int TPC>
 __global__ void __launch_bounds__(KCS_BACK_TPB, PIPE ? 4 : 6) k_back(KGeom g, BackArgs p) {
     const int tid = threadIdx.x;
     const int fg = tid % p.FG;
@@ -465,7 +468,7 @@ __global__ void __launch_bounds__(KCS_BACK_TPB, PIPE ? 4 : 6) k_back(KGeom g, Ba
 #pragma unroll
             for (int f = 0; f < 4; ++f) acc[zb][v][f] = 0.f;
 
-    const int Tp = p.Tp;
+    const int Tp = TPC ? TPC : p.Tp;
     if (p.osl && active) {
         // the epilogue's x and F lines come from HBM (they do not fit L2 between subsets at C4): start them now
 #pragma unroll
@@ -488,29 +491,38 @@ __global__ void __launch_bounds__(KCS_BACK_TPB, PIPE ? 4 : 6) k_back(KGeom g, Ba
         // Software pipeline: the record of angle l+1 is requested before the math of angle l, and the windows of all ZB
         // slices of an angle are requested together, so a thread waits on global memory once per angle, not ZB+1 times
         // (ncu source page of the un-pipelined loop: 16 % of the stall samples on the record, 4 x 5.5 % on the windows).
+        const size_t rstep = (size_t)(p.subset < 0 ? 1 : g.S) * astride;          // record stride from angle to angle
+        const float4 *rec = rec0 + (size_t)(p.subset < 0 ? 0 : p.subset) * astride;  // record of the angle to load next
+        const size_t qstep = (size_t)g.B * Tp;                                      // sinogram row stride from angle to angle
+        const float *ql[ZB];
+#pragma unroll
+        for (int zb = 0; zb < ZB; ++zb) {
+            const int z = min(z0 + zb, g.nz - 1);  // a slice beyond the volume re-reads the last one; its result is dropped
+            ql[zb] = p.qi + (size_t)z * p.As * qstep + fg * 4;
+        }
         float4 n0, n1, n2, n3, n4, n5;
         if (PIPE) {
-            const float4 *rec = rec0 + (size_t)(p.subset < 0 ? 0 : p.subset) * astride;
             n0 = __ldg(rec); n1 = __ldg(rec + 4); n2 = __ldg(rec + 8); n3 = __ldg(rec + 12); n4 = __ldg(rec + 16); n5 = __ldg(rec + 20);
+            rec += rstep;
         }
         for (int l = 0; l < p.As; ++l) {
             if (!PIPE) {
-                const float4 *rec = rec0 + (size_t)(p.subset < 0 ? l : p.subset + l * g.S) * astride;
                 n0 = __ldg(rec); n1 = __ldg(rec + 4); n2 = __ldg(rec + 8); n3 = __ldg(rec + 12); n4 = __ldg(rec + 16); n5 = __ldg(rec + 20);
+                rec += rstep;
             }
             const float4 r0 = n0, r1 = n1, r2 = n2, r3 = n3, r4 = n4, r5 = n5;
             const int base = __float_as_int(r0.x);
             float4 q[ZB][5];
 #pragma unroll
             for (int zb = 0; zb < ZB; ++zb) {
-                const int z = min(z0 + zb, g.nz - 1);  // a slice beyond the volume re-reads the last one; its result is dropped
-                const float *row = p.qi + (((size_t)z * p.As + l) * g.B + base) * Tp + fg * 4;
+                const float *row = ql[zb] + (size_t)base * Tp;
 #pragma unroll
                 for (int r = 0; r < 5; ++r) q[zb][r] = __ldg(reinterpret_cast<const float4 *>(row + r * Tp));
+                ql[zb] += qstep;
             }
             if (PIPE && l + 1 < p.As) {
-                const float4 *rec = rec0 + (size_t)(p.subset < 0 ? l + 1 : p.subset + (l + 1) * g.S) * astride;
                 n0 = __ldg(rec); n1 = __ldg(rec + 4); n2 = __ldg(rec + 8); n3 = __ldg(rec + 12); n4 = __ldg(rec + 16); n5 = __ldg(rec + 20);
+                rec += rstep;
             }
             const float w[4][5] = {{r0.y, r0.z, r0.w, r1.x, r1.y},
                                    {r1.z, r1.w, r2.x, r2.y, r2.z},
@@ -630,9 +642,11 @@ int kcs_launch_back(kcs_ctx *c, int Tp, int subset, int osl, float *out_inner, f
     if (!osl && g.nz >= 2 && (long long)gx * gy * ((g.nz + 1) / 2) >= 148LL) ZB = 2;
     dim3 grid(gx, gy, (g.nz + ZB - 1) / ZB);
     ProfScope ps(c, KCS_K_BACK);
-    if (osl) k_back<1, false><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
-    else if (ZB == 2) k_back<2, true><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
-    else k_back<1, true><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
+    if (osl && Tp == 32) k_back<1, false, 32><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
+    else if (osl) k_back<1, false, 0><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
+    else if (ZB == 2 && Tp == 32) k_back<2, true, 32><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
+    else if (ZB == 2) k_back<2, true, 0><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
+    else k_back<1, true, 0><<<grid, KCS_BACK_TPB, 0, c->stream>>>(g, p);
     LAUNCH_CHECK(c);
     return KCS_OK;
 }
