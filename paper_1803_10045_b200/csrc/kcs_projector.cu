@@ -177,7 +177,10 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, 6) k_forward(KGeom g, FwdArgs p) 
         const int k_lo = (int)ceil(tlo);       // clip bounds were moved 1e-6 steps inwards: strictly inside the margin
         const int k_hi = (int)floor(thi) + 1;
         const int rowstride = g.nxp * Tp;
-        const float *slice = p.xi + (size_t)z * g.nyp * rowstride + fg * FPT;
+        // taps are addressed as (CTA-uniform slice base) + (32-bit byte offset): one IMAD pair per sample instead of 64-bit
+        // pointer arithmetic per tap (a padded slice is < 4 GB)
+        const char *slice = reinterpret_cast<const char *>(p.xi + (size_t)z * g.nyp * rowstride);
+        const unsigned rsb = (unsigned)rowstride * 4u, psb = (unsigned)Tp * 4u, fgb = (unsigned)fg * (FPT * 4u);
         // Anchor blocks sit on the absolute grid k = 0, 16, 32, ...: the fixed-point coordinates of sample k do not depend
         // on where clipping (or the K-split) starts the walk, so a clipped and an unclipped projection of an image that is
         // zero outside the field of view agree bit for bit.
@@ -193,11 +196,12 @@ __global__ void __launch_bounds__(KCS_FWD_TPB, 6) k_forward(KGeom g, FwdArgs p) 
                 const int i0 = fxq >> FB, j0 = fyq >> FB;
                 const float wx = __uint_as_float((((unsigned)fxq & fmask) << msh) | 0x3f800000u) - 1.f;
                 const float wy = __uint_as_float((((unsigned)fyq & fmask) << msh) | 0x3f800000u) - 1.f;
-                const int off = j0 * rowstride + i0 * Tp;
-                const float4 *p00 = reinterpret_cast<const float4 *>(slice + off);
-                const float4 *p01 = reinterpret_cast<const float4 *>(slice + (off + rowstride));
+                const unsigned bo = (unsigned)j0 * rsb + (unsigned)i0 * psb + fgb, bo1 = bo + rsb;
                 const float w11 = wx * wy, w10 = wx - w11, w01 = wy - w11, w00 = (1.f - wx) - w01;
-                const float4 v00 = __ldg(p00), v10 = __ldg(p00 + FG), v01 = __ldg(p01), v11 = __ldg(p01 + FG);
+                const float4 v00 = __ldg(reinterpret_cast<const float4 *>(slice + bo)),
+                             v10 = __ldg(reinterpret_cast<const float4 *>(slice + bo + psb)),
+                             v01 = __ldg(reinterpret_cast<const float4 *>(slice + bo1)),
+                             v11 = __ldg(reinterpret_cast<const float4 *>(slice + bo1 + psb));
                 acc[0] = fmaf(w11, v11.x, fmaf(w01, v01.x, fmaf(w10, v10.x, fmaf(w00, v00.x, acc[0]))));
                 acc[1] = fmaf(w11, v11.y, fmaf(w01, v01.y, fmaf(w10, v10.y, fmaf(w00, v00.y, acc[1]))));
                 acc[2] = fmaf(w11, v11.z, fmaf(w01, v01.z, fmaf(w10, v10.z, fmaf(w00, v00.z, acc[2]))));
