@@ -218,6 +218,33 @@ __global__ void __launch_bounds__(128) k_kinetic(KGeom g, KKin kin, const float 
     }
 }
 
+// The model curve of the ICM path (a1): in-mask voxels only (the OSL update reads F nowhere else; the rest of Fi keeps the
+// zeros it was created with), written to the padded frame-innermost layout four frames at a time (one 16 B store per
+// lane instead of four scattered 4 B stores; frames T..Tp-1 are written as 0).
+__global__ void __launch_bounds__(128) k_kinetic_inner(KGeom g, KKin kin, const float *__restrict__ theta, float *F, long long nvox,
+                                                       const int *__restrict__ vlist, int M2, int Tp) {
+    extern __shared__ double sh_raw[];
+    KFrame *fr = reinterpret_cast<KFrame *>(sh_raw);
+    load_frames(kin, fr);
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)M2 * g.nz) return;
+    const int v2 = g.nx * g.ny;
+    const int z = (int)(t / M2), rem = vlist[(int)(t - (long long)z * M2)];
+    const long long v = (long long)z * v2 + rem;
+    const double K1 = theta[v], k2 = theta[nvox + v], k3 = theta[2 * nvox + v], vB = theta[3 * nvox + v];
+    const XAddr xa = x_addr(g, (size_t)nvox, v, 1, Tp);
+    float4 *dst = reinterpret_cast<float4 *>(F + xa.base);
+    float b0 = 0.f, b1 = 0.f, b2 = 0.f, b3 = 0.f;  // a four-frame shift register (no dynamic register indexing)
+    const int T = kin.T;
+    tac_stream<false>(kin, fr, K1, k2, k3, vB, [&](int m, double Fm, double, double, double, double) {
+        b0 = b1; b1 = b2; b2 = b3; b3 = (float)Fm;
+        if (m == T - 1)
+            for (int pad = 3 - (m & 3); pad > 0; --pad) { b0 = b1; b1 = b2; b2 = b3; b3 = 0.f; }  // the last, partial group
+        if ((m & 3) == 3 || m == T - 1) dst[m >> 2] = make_float4(b0, b1, b2, b3);
+    });
+    for (int q = (T + 3) / 4; q < Tp / 4; ++q) dst[q] = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // MAP-LM step (L1-L3).  One thread = one voxel; everything per-voxel lives in fp64 registers.
 // ---------------------------------------------------------------------------------------------------------
@@ -432,7 +459,12 @@ int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int i
     const long long nvox = (long long)c->n_vox;
     const size_t smem = sizeof(KFrame) * c->kin.T;
     ProfScope ps(c, KCS_K_KINETIC);
-    k_kinetic<<<(unsigned)((nvox + 127) / 128), 128, smem, c->stream>>>(c->g, c->kin, theta, F, J, nvox, inner, Tp);
+    if (inner && !J) {
+        const long long nfit = (long long)c->n_inmask2 * c->g.nz;
+        if (nfit > 0)
+            k_kinetic_inner<<<(unsigned)((nfit + 127) / 128), 128, smem, c->stream>>>(c->g, c->kin, theta, F, nvox, c->d_vlist, c->n_inmask2, Tp);
+    } else
+        k_kinetic<<<(unsigned)((nvox + 127) / 128), 128, smem, c->stream>>>(c->g, c->kin, theta, F, J, nvox, inner, Tp);
     LAUNCH_CHECK(c);
     return KCS_OK;
 }
