@@ -32,48 +32,44 @@ struct PackMap {
     int off;         // dst pixel offset of (row 0, col 0) inside a slab
 };
 
-__device__ __forceinline__ long long pack_dst(const PackMap &m, long long row, int col) {
-    return (row / m.rps) * m.slab + (long long)(row % m.rps) * m.rstride + m.off + col;
+// rows and slabs fit 32 bits (kcs_launch_pack checks); Tp is a power of two (round_up4), lt = log2(Tp)
+__device__ __forceinline__ size_t pack_dst(const PackMap &m, unsigned row, int col) {
+    const unsigned s = row / (unsigned)m.rps, rr = row - s * (unsigned)m.rps;
+    return (size_t)s * (size_t)m.slab + (size_t)rr * m.rstride + m.off + col;
 }
 
 // block (32, 8): one row segment of 32 columns, all frames.
-__global__ void k_pack(const float *__restrict__ src, size_t fs, int nf, float *__restrict__ dst, int Tp, PackMap m) {
+__global__ void __launch_bounds__(256) k_pack(const float *__restrict__ src, size_t fs, int nf, float *__restrict__ dst, int Tp, int lt,
+                                              PackMap m) {
     __shared__ float tile[KCS_MAX_FRAMES][33];
     const int c0 = blockIdx.x * 32;
-    const long long row = blockIdx.y + (long long)blockIdx.z * gridDim.y;
-    if (row >= m.nrows) return;
+    const unsigned row = blockIdx.y + blockIdx.z * gridDim.y;
+    if (row >= (unsigned)m.nrows) return;
     const int tx = threadIdx.x, ty = threadIdx.y;
-    for (int f = ty; f < Tp; f += 8) {
-        float v = 0.f;
-        if (f < nf && c0 + tx < m.W) v = src[(size_t)f * fs + (size_t)row * m.W + c0 + tx];
-        tile[f][tx] = v;
-    }
+    const float *sp = src + (size_t)row * m.W + c0 + tx;
+    for (int f = ty; f < Tp; f += 8) tile[f][tx] = (f < nf && c0 + tx < m.W) ? sp[(size_t)f * fs] : 0.f;
     __syncthreads();
     const int ncol = min(32, m.W - c0);
-    const long long d0 = pack_dst(m, row, c0);
-    const int n = ncol * Tp;
-    for (int e = ty * 32 + tx; e < n; e += 256) {
-        const int col = e / Tp, f = e - col * Tp;
-        dst[(size_t)d0 * Tp + e] = tile[f][col];
-    }
+    float *dp = dst + pack_dst(m, row, c0) * Tp;
+    const int n = ncol << lt;
+    for (int e = ty * 32 + tx; e < n; e += 256) dp[e] = tile[e & (Tp - 1)][e >> lt];
 }
 
-__global__ void k_unpack(const float *__restrict__ src, int Tp, float *__restrict__ dst, size_t fs, int nf, PackMap m) {
+__global__ void __launch_bounds__(256) k_unpack(const float *__restrict__ src, int Tp, int lt, float *__restrict__ dst, size_t fs, int nf,
+                                                PackMap m) {
     __shared__ float tile[KCS_MAX_FRAMES][33];
     const int c0 = blockIdx.x * 32;
-    const long long row = blockIdx.y + (long long)blockIdx.z * gridDim.y;
-    if (row >= m.nrows) return;
+    const unsigned row = blockIdx.y + blockIdx.z * gridDim.y;
+    if (row >= (unsigned)m.nrows) return;
     const int tx = threadIdx.x, ty = threadIdx.y;
     const int ncol = min(32, m.W - c0);
-    const long long d0 = pack_dst(m, row, c0);
-    const int n = ncol * Tp;
-    for (int e = ty * 32 + tx; e < n; e += 256) {
-        const int col = e / Tp, f = e - col * Tp;
-        tile[f][col] = src[(size_t)d0 * Tp + e];
-    }
+    const float *sp = src + pack_dst(m, row, c0) * Tp;
+    const int n = ncol << lt;
+    for (int e = ty * 32 + tx; e < n; e += 256) tile[e & (Tp - 1)][e >> lt] = sp[e];
     __syncthreads();
-    for (int f = ty; f < nf; f += 8)
-        if (c0 + tx < m.W) dst[(size_t)f * fs + (size_t)row * m.W + c0 + tx] = tile[f][tx];
+    float *dp = dst + (size_t)row * m.W + c0 + tx;
+    if (c0 + tx < m.W)
+        for (int f = ty; f < nf; f += 8) dp[(size_t)f * fs] = tile[f][tx];
 }
 
 static void pack_grid(long long nrows, int W, dim3 &grid) {
@@ -83,22 +79,28 @@ static void pack_grid(long long nrows, int W, dim3 &grid) {
 
 int kcs_launch_pack(kcs_ctx *c, const float *src, size_t fs, int nf, float *dst, int Tp, long long nrows, int W,
                     int rps, long long slab, int rstride, int off) {
+    if (nrows >= (1LL << 31)) { c->err = "kcs_launch_pack: more than 2^31 rows"; return KCS_ERR_SHAPE; }
     PackMap m{nrows, W, rps, slab, rstride, off};
     dim3 grid;
     pack_grid(nrows, W, grid);
     ProfScope ps(c, KCS_K_PACK);
-    k_pack<<<grid, dim3(32, 8), 0, c->stream>>>(src, fs, nf, dst, Tp, m);
+    int lt = 2;
+    while ((1 << lt) < Tp) ++lt;
+    k_pack<<<grid, dim3(32, 8), 0, c->stream>>>(src, fs, nf, dst, Tp, lt, m);
     LAUNCH_CHECK(c);
     return KCS_OK;
 }
 
 int kcs_launch_unpack(kcs_ctx *c, const float *src, int Tp, float *dst, size_t fs, int nf, long long nrows, int W,
                       int rps, long long slab, int rstride, int off) {
+    if (nrows >= (1LL << 31)) { c->err = "kcs_launch_unpack: more than 2^31 rows"; return KCS_ERR_SHAPE; }
     PackMap m{nrows, W, rps, slab, rstride, off};
     dim3 grid;
     pack_grid(nrows, W, grid);
     ProfScope ps(c, KCS_K_UNPACK);
-    k_unpack<<<grid, dim3(32, 8), 0, c->stream>>>(src, Tp, dst, fs, nf, m);
+    int lt = 2;
+    while ((1 << lt) < Tp) ++lt;
+    k_unpack<<<grid, dim3(32, 8), 0, c->stream>>>(src, Tp, lt, dst, fs, nf, m);
     LAUNCH_CHECK(c);
     return KCS_OK;
 }
