@@ -447,7 +447,7 @@ int kcs_launch_build_wtab(kcs_ctx *c) {
 //               (x and F from HBM) overlaps other CTAs' angle loops better at 24 warps per SM (2.50 ms against 2.64).
 // TPC: the padded frame count as a compile-time constant (32 on the ICM path of C2-C4: the window loads then take immediate
 // offsets) or 0 for "read p.Tp".  Record and row pointers advance by constant strides from angle to angle; the loop body of
-// <1, false, 32> went from 150 to SASS instructions per angle for 80 FFMA with both.
+// <1, false, 32> went from 150 to 106 SASS instructions per angle for 80 FFMA with both.
 template <int ZB, bool PIPE, int TPC>
 __global__ void __launch_bounds__(KCS_BACK_TPB, PIPE ? 4 : 6) k_back(KGeom g, BackArgs p) {
     const int tid = threadIdx.x;
