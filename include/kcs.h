@@ -192,6 +192,30 @@ int kcs_icm_run_host(kcs_ctx *ctx, const float *y, const float *r, int r_mode, f
                      float *x, float *theta, float *lambda,
                      float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter);
 
+/* ---- the one entry point that allocates nothing ------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): kcs_forward_project (P1-P3, the projection sum of eq. 2's denominator) WITHOUT a kcs_ctx.  It calls no
+ * cudaMalloc, cudaFree or allocating library routine: the packed volume, the packed sinogram and the angle table --
+ * the workspace kcs_create would allocate -- sit in one static __device__ array of KCS_STATIC_SCRATCH_BYTES inside the
+ * library (every GPU this entry point has run on holds that much until the process exits).  The kernels and the
+ * arithmetic are those of kcs_forward_project: same result for the same cfg geometry.
+ *   cfg     [host] only the geometry is read: nx, ny, nz, vx, vy, n_angles, n_bins, bin_mm, n_steps, step_mm,
+ *           n_subsets (frame tables, input function, mask and n_replicas are ignored)
+ *   x       [device] nf frames [nf][nz][ny][nx];   y_s [device] out, [nf][nz][As][B], As = A (subset = -1) or A/S
+ *   nf      1..KCS_MAX_FRAMES;   stream = the CUDA stream (of the CURRENT device) the work is enqueued on, no sync
+ * LIMIT: 256-rounded bytes of  16*2 A  +  4 Tp nz (ny+4)(nx+4)  +  4 Tp nz As B  <= KCS_STATIC_SCRATCH_BYTES
+ * (Tp = power of two >= nf, 4..32; BJ configs[0] and [1] fit, configs[2] and [3] do not): a larger problem is rejected
+ * with KCS_ERR_SHAPE before any CUDA call, and kcs_static_last_error() says how many bytes it needed.
+ * SHARING: every call on a device uses the same array, which keeps the last call's contents (the part that must start
+ * at zero is cleared by every call); two calls that overlap on the GPU (different streams, or graphs replayed
+ * concurrently) RACE -- order them on one stream or with events.  The first call on a device takes the array's address
+ * (cudaGetSymbolAddress, which may load the module): make it outside stream capture.
+ * Errors: KCS_ERR_NULL / _SHAPE / _SUBSET / _FRAMES / _CUDA as above; message (per host thread) from
+ * kcs_static_last_error(). */
+#define KCS_STATIC_SCRATCH_BYTES (40u << 20) /* 40 MiB */
+int kcs_forward_project_static(const kcs_config *cfg, const float *x, float *y_s, int subset, int nf, void *stream);
+const char *kcs_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -32,7 +32,8 @@ PROFILE_CLASSES = ("pack", "unpack", "kinetic", "forward", "back", "lm", "other"
 # every symbol include/kcs.h declares (tests/test_abi.py checks the library exports each of them)
 EXPORTS = ["kcs_create", "kcs_destroy", "kcs_set_stream", "kcs_last_error", "kcs_workspace_bytes", "kcs_get_mask",
            "kcs_launch_count", "kcs_use_graphs", "kcs_graph_replays", "kcs_profile_enable", "kcs_profile_read", "kcs_forward_project", "kcs_back_project", "kcs_sensitivity", "kcs_osl_update",
-           "kcs_kinetic_eval", "kcs_ki_map", "kcs_set_multiplicative", "kcs_set_fit_options", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host"]
+           "kcs_kinetic_eval", "kcs_ki_map", "kcs_set_multiplicative", "kcs_set_fit_options", "kcs_map_lm", "kcs_icm_iteration", "kcs_icm_run", "kcs_icm_run_host",
+           "kcs_forward_project_static", "kcs_static_last_error"]
 
 
 class KcsError(RuntimeError):
@@ -107,8 +108,35 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.kcs_icm_iteration.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, i]
     lib.kcs_icm_run.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, f, i, i]
     lib.kcs_icm_run_host.argtypes = [vp, fp, fp, i, f, fp, fp, fp, f, f, f, f, i, i]
+    lib.kcs_forward_project_static.argtypes = [C.POINTER(_Config), fp, fp, i, i, vp]
+    lib.kcs_static_last_error.argtypes = []
+    lib.kcs_static_last_error.restype = C.c_char_p
     _lib = lib
     return lib
+
+
+STATIC_SCRATCH_BYTES = 40 << 20  # KCS_STATIC_SCRATCH_BYTES of include/kcs.h
+
+
+def forward_project_static(cfg: dict, x, y_s, subset: int = -1, stream=None):
+    """kcs_forward_project_static: the forward projector without a Context and without any device allocation (its
+    workspace is a static 40 MiB device array inside libkcs.so; larger geometries raise KCS_ERR_SHAPE).
+    x [nf, nz, ny, nx] -> y_s [nf, nz, As, B] on `stream` (default: torch's current stream).  Calls share the array:
+    calls that overlap on the GPU race."""
+    lib = load()
+    c = _Config()
+    for k in ("nx", "ny", "nz", "n_angles", "n_bins", "n_steps", "n_subsets"):
+        setattr(c, k, int(cfg[k]))
+    for k in ("vx", "vy", "vz", "bin_mm", "step_mm"):
+        setattr(c, k, float(cfg[k]))
+    nf = int(x.shape[0])
+    As = c.n_angles if subset < 0 else c.n_angles // max(c.n_subsets, 1)
+    px, py = _dev(x, (nf, c.nz, c.ny, c.nx)), _dev(y_s, (nf, c.nz, As, c.n_bins))
+    if stream is None:
+        stream = _torch().cuda.current_stream().cuda_stream
+    rc = lib.kcs_forward_project_static(C.byref(c), px, py, int(subset), nf, C.c_void_p(stream))
+    if rc != KCS_OK:
+        raise KcsError(rc, lib.kcs_static_last_error().decode())
 
 
 def probe_peak(what: str, stream=None) -> float:

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(HERE, "..", "include")
 LIB = os.path.join(HERE, "libkcs.so")
-SOURCES = ["kcs_api.cu", "kcs_projector.cu", "kcs_kinetic.cu"]
+SOURCES = ["kcs_api.cu", "kcs_projector.cu", "kcs_kinetic.cu", "kcs_static.cu"]
 HEADERS = [os.path.join(CSRC, "kcs_internal.cuh"), os.path.join(INC, "kcs.h")]
 PROBE_LIB = os.path.join(HERE, "libkcs_probe.so")
 PROBE_SOURCES = [os.path.join("bench", "kcs_probe.cu")]
