@@ -221,10 +221,11 @@ int kcs_destroy(kcs_ctx *c) {
     for (KGraphEntry &ge : c->graphs) cudaGraphExecDestroy(ge.exec);
     for (const KProfRec &r : c->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (cudaEvent_t e : c->prof_pool) cudaEventDestroy(e);
-    if (c->in_stream) { cudaStreamDestroy(c->in_stream); cudaStreamDestroy(c->out_stream); cudaEventDestroy(c->ev_small); }
+    if (c->in_stream) { cudaStreamDestroy(c->in_stream); cudaStreamDestroy(c->out_stream); cudaEventDestroy(c->ev_small); cudaEventDestroy(c->ev_lam); }
     for (cudaEvent_t e : c->ev_in) cudaEventDestroy(e);
     for (cudaEvent_t e : c->ev_out) cudaEventDestroy(e);
     if (c->aux_stream) { cudaStreamDestroy(c->aux_stream); cudaEventDestroy(c->ev_fork); cudaEventDestroy(c->ev_join); }
+    if (c->os_stream) { cudaStreamDestroy(c->os_stream); cudaEventDestroy(c->ev_os_fork); cudaEventDestroy(c->ev_os_join); }
     delete c;
     return KCS_OK;
 }
@@ -264,8 +265,9 @@ int kcs_create(kcs_ctx **out, const kcs_config *cfg, void *stream) {
     c->xi = c->Fi = c->qi = c->yi = c->ri = c->r_pad = c->theta2 = nullptr;
     c->thD[0] = c->thD[1] = c->lamD = nullptr;
     c->lm_state = nullptr;
-    c->in_stream = c->out_stream = nullptr; c->ev_small = nullptr;
+    c->in_stream = c->out_stream = nullptr; c->ev_small = c->ev_lam = nullptr;
     c->aux_stream = nullptr; c->ev_fork = c->ev_join = nullptr;
+    c->os_stream = nullptr; c->ev_os_fork = c->ev_os_join = nullptr;
     c->st_y = c->st_r = c->st_x = c->st_theta = c->st_lambda = nullptr;
     c->st_r_elems = 0;
 
@@ -596,16 +598,36 @@ static int start_kinetic(kcs_ctx *c, const float *theta, int Tp) {
 }
 
 // Host-buffer mode of the ICM loop (kcs_icm_run_host): y and x arrive from / x returns to HOST memory in z chunks.
+#define KCS_MAX_CHUNKS 9
 struct HostIO {
     const float *hy;   // [host] y[T][nz][A][B]
     float *hx;         // [host] x[T][nz][ny][nx], in and out
     int nchunk;
+    int zb[KCS_MAX_CHUNKS + 1];  // chunk k = slices [zb[k], zb[k + 1])
+    cudaEvent_t ev_lam;          // lambda (copied in last: only MAP-LM reads it) is on the device
 };
 
-static void chunk_range(const KGeom &g, int nchunk, int k, int &z0, int &nzc) {
-    const int per = (g.nz + nchunk - 1) / nchunk;
-    z0 = k * per;
-    nzc = z0 >= g.nz ? 0 : (z0 + per > g.nz ? g.nz - z0 : per);
+// The z chunks of the host-buffer pipeline.  Nothing can run before the first chunk has arrived, and the last chunk's x
+// leaves behind MAP-LM anyway: the LEAD chunk is the smallest that fills the GPU once (148 SMs x 6 forward CTAs of 128
+// ray lanes), each following chunk is twice the one before (the OS pass of a slice takes about twice its copy), up to a
+// quarter of the volume (>= 16 slices); a remainder of less than half a chunk joins the last one.
+static void plan_chunks(const kcs_ctx *c, HostIO &io) {
+    const KGeom &g = c->g;
+    const double lanes_per_slice = (double)(g.A / g.S) * g.B * (round_up4(c->cfg.n_frames) / 4);
+    int s = (int)std::ceil(148.0 * 6 * 128 / lanes_per_slice);
+    if (s < 1) s = 1;
+    const int cap = (g.nz + 3) / 4 > 16 ? (g.nz + 3) / 4 : 16;
+    if (s > cap) s = cap;
+    int k = 0, z = 0;
+    io.zb[0] = 0;
+    while (z < g.nz) {
+        int take = s < g.nz - z ? s : g.nz - z;
+        if (k == KCS_MAX_CHUNKS - 1 || g.nz - z - take < (take + 1) / 2) take = g.nz - z;
+        z += take;
+        io.zb[++k] = z;
+        s = 2 * s < cap ? 2 * s : cap;
+    }
+    io.nchunk = k;
 }
 
 // The ICM loop.  y, x: DEVICE buffers (the caller's, or the staging buffers of kcs_icm_run_host when io != NULL).
@@ -621,7 +643,26 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
     if (n_lm < 0 || n_iter < 0 || !(scale > 0.f)) return fail(c, KCS_ERR_SHAPE, "kcs_icm: bad n_lm / n_iter / scale");
     const KGeom &g = c->g;
     const int T = c->cfg.n_frames, Tp = round_up4(T);
+    // Host-buffer mode: two LANES (the context's stream and a second one) carry the OS pass of alternate z chunks.  Direct
+    // planes are independent, and while one chunk's kernel drains its last CTAs the other chunk's kernel fills the SMs: a
+    // chunk launch ends in a tail of ~0.1 ms, 42 times per chunk and iteration.  (A device-resident call is one chunk on
+    // the context's stream: split in two halves the C4 iteration gains 1 %, and per-kernel timing wants kernels that have
+    // the GPU to themselves.)
+    const bool two = io != nullptr && io->nchunk >= 2 && !c->prof_on;
+    const int whole[2] = {0, g.nz};
     const int nchunk = io ? io->nchunk : 1;
+    const int *zb = io ? io->zb : whole;
+    const int nlane = two ? 2 : 1;
+    if (two && !c->os_stream) {
+        KCS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->os_stream, cudaStreamNonBlocking));
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_os_fork, cudaEventDisableTiming));
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_os_join, cudaEventDisableTiming));
+    }
+    struct StreamRestore {  // the launchers enqueue on c->stream: it is switched per chunk and put back on every exit
+        kcs_ctx *c; cudaStream_t s;
+        ~StreamRestore() { c->stream = s; }
+    } restore{c, c->stream};
+    cudaStream_t lanes[2] = {c->stream, c->os_stream};
     int rc;
     if (n_iter > 0 && (rc = start_kinetic(c, theta, Tp))) return rc;  // beside the packing and the first forward projection
     if ((rc = ensure_border(c, Tp))) return rc;
@@ -645,10 +686,16 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
         const float b = it == 0 ? beta_first : beta;
         const bool last = it == n_iter - 1;
         if (it > 0 && (rc = start_kinetic(c, theta, Tp))) return rc;
+        if (two) {  // lane 1 starts behind everything enqueued so far (packing, the previous iteration's MAP-LM)
+            KCS_CUDA_OK(c, cudaEventRecord(c->ev_os_fork, lanes[0]));
+            KCS_CUDA_OK(c, cudaStreamWaitEvent(lanes[1], c->ev_os_fork, 0));
+        }
+        bool has_F[2] = {false, false};
         for (int k = 0; k < nchunk; ++k) {
-            int z0, nzc;
-            chunk_range(g, nchunk, k, z0, nzc);
+            const int z0 = zb[k], nzc = zb[k + 1] - zb[k];
             if (nzc == 0) continue;
+            const int lane = k % nlane;
+            c->stream = lanes[lane];
             if (io && it == 0) {  // this chunk's x and y have been copied to the staging buffers: pack them
                 KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_in[k], 0));
                 if ((rc = pack_image(c, x, T, c->xi, Tp, z0, nzc))) return rc;
@@ -657,13 +704,21 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
             for (int s = 0; s < g.S; ++s) {  // Q5: subsets in order 0..S-1
                 // after the first OSL update of this call x is zero outside the mask: rays are clipped to the FOV circle
                 if ((rc = kcs_launch_forward(c, Tp, s, 1, scale, r_mode, (it > 0 || s > 0) ? 1 : 0, z0, nzc))) return rc;
-                if (s == 0 && k == 0) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
+                if (!has_F[lane]) {  // the model curve (second stream) is needed from the first OSL update on
+                    KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
+                    has_F[lane] = true;
+                }
                 if ((rc = kcs_launch_back(c, Tp, s, 1, nullptr, scale, b, z0, nzc))) return rc;
             }
             if (io && last) {  // this chunk's activity is final: unpack it and let the copy-out stream take it
                 if ((rc = unpack_image(c, c->xi, Tp, x, T, z0, nzc))) return rc;
                 KCS_CUDA_OK(c, cudaEventRecord(c->ev_out[k], c->stream));
             }
+        }
+        c->stream = lanes[0];
+        if (two) {
+            KCS_CUDA_OK(c, cudaEventRecord(c->ev_os_join, lanes[1]));
+            KCS_CUDA_OK(c, cudaStreamWaitEvent(lanes[0], c->ev_os_join, 0));
         }
         if (last && !io) {  // the activity is final after the last OS pass; MAP-LM only reads it: unpack beside the fit
             cudaStream_t main_stream = c->stream;
@@ -675,6 +730,7 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
             if (rc) return rc;
             KCS_CUDA_OK(c, cudaEventRecord(c->ev_join, c->aux_stream));
         }
+        if (io && it == 0) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, io->ev_lam, 0));
         if ((rc = lm_steps(c, c->xi, 1, Tp, theta, lambda, gamma, delta, n_lm, nullptr))) return rc;
         if (last && !io) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
     }
@@ -796,13 +852,16 @@ int kcs_icm_run_host(kcs_ctx *c, const float *y, const float *r, int r_mode, flo
         cudaGetLastError();
         return fail(c, KCS_ERR_ALLOC, std::string("kcs_icm_run_host: ") + cudaGetErrorString(e));
     }
-    // z chunks of >= 16 slices, at most 8 of them: big enough to fill the GPU, small enough to hide the copies
-    HostIO io{y, x, g.nz / 16 < 1 ? 1 : (g.nz / 16 > 8 ? 8 : g.nz / 16)};
+    HostIO io{};
+    io.hy = y; io.hx = x;
+    plan_chunks(c, io);
     if (!c->in_stream) {
         KCS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->in_stream, cudaStreamNonBlocking));
         KCS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->out_stream, cudaStreamNonBlocking));
         KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_small, cudaEventDisableTiming));
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_lam, cudaEventDisableTiming));
     }
+    io.ev_lam = c->ev_lam;
     while ((int)c->ev_in.size() < io.nchunk) {
         cudaEvent_t a = nullptr, b = nullptr;
         KCS_CUDA_OK(c, cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
@@ -815,13 +874,12 @@ int kcs_icm_run_host(kcs_ctx *c, const float *y, const float *r, int r_mode, flo
     // may still be in use by a previous call)
     KCS_CUDA_OK(c, cudaEventRecord(c->ev_small, st));
     KCS_CUDA_OK(c, cudaStreamWaitEvent(in, c->ev_small, 0));
+    // order on the copy-in stream: theta and r (the model curve and the first ratio need them), the chunks, lambda last
     KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_theta, theta, 4 * c->n_vox * sizeof(float), cudaMemcpyHostToDevice, in));
-    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_lambda, lambda, c->n_vox * sizeof(float), cudaMemcpyHostToDevice, in));
     KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_r, r, nr * sizeof(float), cudaMemcpyHostToDevice, in));
     KCS_CUDA_OK(c, cudaEventRecord(c->ev_small, in));
     for (int k = 0; k < io.nchunk; ++k) {  // x and y of chunk k: T strided pieces each (one 2-D copy)
-        int z0, nzc;
-        chunk_range(g, io.nchunk, k, z0, nzc);
+        const int z0 = io.zb[k], nzc = io.zb[k + 1] - io.zb[k];
         if (nzc > 0) {
             const size_t v2 = (size_t)g.ny * g.nx, r2 = (size_t)g.A * g.B;
             KCS_CUDA_OK(c, cudaMemcpy2DAsync(c->st_x + z0 * v2, c->n_vox * sizeof(float), x + z0 * v2, c->n_vox * sizeof(float),
@@ -831,16 +889,19 @@ int kcs_icm_run_host(kcs_ctx *c, const float *y, const float *r, int r_mode, flo
         }
         KCS_CUDA_OK(c, cudaEventRecord(c->ev_in[k], in));
     }
+    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_lambda, lambda, c->n_vox * sizeof(float), cudaMemcpyHostToDevice, in));
+    KCS_CUDA_OK(c, cudaEventRecord(c->ev_lam, in));
     KCS_CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_small, 0));
-    if (n_iter <= 0)  // nothing to overlap: wait for every chunk, the loop below only unpacks
+    if (n_iter <= 0) {  // nothing to overlap: wait for every chunk, the loop below only unpacks
         for (int k = 0; k < io.nchunk; ++k) KCS_CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_in[k], 0));
+        KCS_CUDA_OK(c, cudaStreamWaitEvent(st, c->ev_lam, 0));
+    }
     int rc = icm_run_impl(c, c->st_y, c->st_r, r_mode, scale, c->st_x, c->st_theta, c->st_lambda, beta_first, beta, gamma, delta,
                           n_lm, n_iter, n_iter > 0 ? &io : nullptr);
     if (rc) return rc;
     if (n_iter > 0) {
         for (int k = 0; k < io.nchunk; ++k) {  // x of chunk k goes back while later chunks and the last MAP-LM still run
-            int z0, nzc;
-            chunk_range(g, io.nchunk, k, z0, nzc);
+            const int z0 = io.zb[k], nzc = io.zb[k + 1] - io.zb[k];
             if (nzc == 0) continue;
             const size_t v2 = (size_t)g.ny * g.nx;
             KCS_CUDA_OK(c, cudaStreamWaitEvent(out, c->ev_out[k], 0));

@@ -134,10 +134,12 @@ struct kcs_ctx {
     size_t st_r_elems;
     cudaStream_t aux_stream;   // kcs_icm_run: the kinetic evaluator runs here beside the first forward projection
     cudaEvent_t ev_fork, ev_join;
+    cudaStream_t os_stream;    // second lane of the OS pass (alternate z chunks; kcs_api.cu, icm_run_impl)
+    cudaEvent_t ev_os_fork, ev_os_join;
     // kcs_icm_run_host: the volume moves in z chunks; chunk k + 1 is copied in (in_stream) and chunk k - 1 copied out
     // (out_stream) while chunk k goes through its OS pass on the context's stream
     cudaStream_t in_stream, out_stream;
-    cudaEvent_t ev_small;                  // theta, lambda, r are on the device
+    cudaEvent_t ev_small, ev_lam;          // theta and r / lambda are on the device
     std::vector<cudaEvent_t> ev_in, ev_out;  // per chunk: inputs have arrived / x is final on the device
 };
 

@@ -413,6 +413,31 @@ def test_host_entry_moves_the_volume_in_z_chunks():
     ctx.close()
 
 
+def test_host_entry_lead_chunk_and_two_lanes():
+    """With slices as large as C4's (344 x 344, 252 x 344, T = 29) the host pipeline starts with a short lead chunk (4
+    slices), doubles the chunk size from there (8, then the remaining 20 of 32) and runs alternate chunks on two
+    streams: still kcs_icm_run bit for bit.  Inputs: seeded noise, no oracle needed for an equality."""
+    cfg = dict(ki.config("C4"), nz=32)
+    ctx = _kcs().Context(cfg)
+    T, nz, ny, nx, A, B = cfg["n_frames"], 32, cfg["ny"], cfg["nx"], cfg["n_angles"], cfg["n_bins"]
+    mask = ctx.mask()
+    y0 = np.float32(np.floor(4.0 * ki.uniform((T, nz, A, B), seed=61)))
+    r0 = np.float32(0.05 + 0.01 * np.arange(T))
+    x0 = np.float32((0.5 + ki.uniform((T, nz, ny, nx), seed=62)) * mask)
+    th0 = np.float32(np.broadcast_to(np.array([0.1, 0.1, 0.05, 0.05])[:, None, None, None], (4, nz, ny, nx))
+                     * (0.8 + 0.4 * ki.uniform((4, nz, ny, nx), seed=63)))
+    lam0 = np.zeros((nz, ny, nx), dtype=np.float32)
+    for n_iter in (1, 2):
+        x, th, lam = dev(x0), dev(th0), dev(lam0)
+        ctx.icm_run(dev(y0), dev(r0), 1.0, x, th, lam, 0.0, cfg["beta"], cfg["gamma"], cfg["delta"], 2, n_iter)
+        hx, hth, hlam = x0.copy(), th0.copy(), lam0.copy()
+        ctx.icm_run_host(y0, r0, 1.0, hx, hth, hlam, 0.0, cfg["beta"], cfg["gamma"], cfg["delta"], 2, n_iter)
+        assert np.isfinite(hx).all() and float(np.abs(hx).max()) > 0
+        assert np.array_equal(hx, x.cpu().numpy()) and np.array_equal(hth, th.cpu().numpy())
+        assert np.array_equal(hlam, lam.cpu().numpy())
+    ctx.close()
+
+
 def test_projector_C2_full_size():
     """C2 geometry (128x128x8, 120x128, T = 24): several blocks per slice and z-batching in the back-projector."""
     cfg = CONFIGS["C2"]()
