@@ -186,9 +186,10 @@ int kcs_icm_run(kcs_ctx *ctx, const float *y, const float *r, int r_mode, float 
                 float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter);
 
 /* Host-buffer convenience for end-to-end timing: all data pointers [host] (pinned or pageable); copies
- * y, r, x, theta, lambda to the device, runs kcs_icm_run, copies x, theta, lambda back and synchronises.  x and y move
- * in z chunks on library-owned copy streams beside the OS pass of earlier chunks (alternate chunks on the context's
- * stream and a second library-owned one); same result as kcs_icm_run, bit for bit. */
+ * y, r, x, theta, lambda to the device, runs kcs_icm_run, copies x, theta, lambda back and synchronises.  x, y and theta
+ * move in z chunks on library-owned copy streams beside the OS pass of earlier chunks (alternate chunks on the context's
+ * stream and a second library-owned one), theta and lambda return beside the last MAP-LM step; same result as
+ * kcs_icm_run, bit for bit. */
 int kcs_icm_run_host(kcs_ctx *ctx, const float *y, const float *r, int r_mode, float scale,
                      float *x, float *theta, float *lambda,
                      float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter);

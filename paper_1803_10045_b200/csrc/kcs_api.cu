@@ -224,6 +224,7 @@ int kcs_destroy(kcs_ctx *c) {
     if (c->in_stream) { cudaStreamDestroy(c->in_stream); cudaStreamDestroy(c->out_stream); cudaEventDestroy(c->ev_small); cudaEventDestroy(c->ev_lam); }
     for (cudaEvent_t e : c->ev_in) cudaEventDestroy(e);
     for (cudaEvent_t e : c->ev_out) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->ev_lm) cudaEventDestroy(e);
     if (c->aux_stream) { cudaStreamDestroy(c->aux_stream); cudaEventDestroy(c->ev_fork); cudaEventDestroy(c->ev_join); }
     if (c->os_stream) { cudaStreamDestroy(c->os_stream); cudaEventDestroy(c->ev_os_fork); cudaEventDestroy(c->ev_os_join); }
     delete c;
@@ -513,8 +514,24 @@ int kcs_kinetic_eval(kcs_ctx *c, const float *theta, float *F, float *J) {
 
 // n_steps Jacobi steps.  The first reads the caller's fp32 maps, the last writes them; in between the iterate lives
 // in the context's fp64 ping-pong buffers, so a call rounds theta and lambda to fp32 once, not once per step.
+// Host-buffer mode of the ICM loop (kcs_icm_run_host): y, x and theta arrive from / x, theta, lambda return to HOST memory in
+// z ranges.
+#define KCS_MAX_CHUNKS 9
+#define KCS_LM_PIECES 4
+struct HostIO {
+    const float *hy;   // [host] y[T][nz][A][B]
+    float *hx;         // [host] x[T][nz][ny][nx], in and out
+    int nchunk;
+    int zb[KCS_MAX_CHUNKS + 1];  // chunk k = slices [zb[k], zb[k + 1])
+    cudaEvent_t ev_lam;          // lambda (copied in last: only MAP-LM reads it) is on the device
+    // the last MAP-LM step of the call runs in z pieces, so that theta and lambda of a piece leave while the next is fitted
+    int n_piece;                 // set by lm_steps: 0 = the step was not split
+    int pzb[KCS_LM_PIECES + 1];
+    cudaEvent_t ev_lm[KCS_LM_PIECES];
+};
+
 static int lm_steps(kcs_ctx *c, const float *x, int x_inner, int Tp, float *theta, float *lambda, float gamma, float delta,
-                    int n_steps, float *cost) {
+                    int n_steps, float *cost, HostIO *io = nullptr) {
     const size_t map_bytes = 4 * c->n_vox * sizeof(float);
     if (cost) KCS_CUDA_OK(c, cudaMemsetAsync(cost, 0, c->n_vox * sizeof(float), c->stream));  // out-of-mask voxels: 0
     if (n_steps == 1) {  // fp32 scratch pre-filled with the caller's maps: the kernel only writes in-mask voxels
@@ -530,6 +547,17 @@ static int lm_steps(kcs_ctx *c, const float *x, int x_inner, int Tp, float *thet
         void *tout = last ? (void *)theta : (void *)c->thD[s & 1];
         const void *lin = first ? (const void *)lambda : (const void *)c->lamD;
         void *lout = last ? (void *)lambda : (void *)c->lamD;
+        if (last && io && c->g.nz >= KCS_LM_PIECES) {  // Jacobi: the step reads tin only, z pieces are independent launches
+            io->n_piece = KCS_LM_PIECES;
+            for (int p = 0; p <= KCS_LM_PIECES; ++p) io->pzb[p] = (int)((long long)c->g.nz * p / KCS_LM_PIECES);
+            for (int p = 0; p < KCS_LM_PIECES; ++p) {
+                int rc = kcs_launch_lm_step(c, x, x_inner, Tp, tin, 1, tout, 0, lin, lout, gamma, delta, cost, io->pzb[p],
+                                            io->pzb[p + 1] - io->pzb[p]);
+                if (rc) return rc;
+                KCS_CUDA_OK(c, cudaEventRecord(io->ev_lm[p], c->stream));
+            }
+            continue;
+        }
         int rc = kcs_launch_lm_step(c, x, x_inner, Tp, tin, first ? 0 : 1, tout, last ? 0 : 1, lin, lout, gamma, delta,
                                     last ? cost : nullptr);
         if (rc) return rc;
@@ -597,16 +625,6 @@ static int start_kinetic(kcs_ctx *c, const float *theta, int Tp) {
     return KCS_OK;
 }
 
-// Host-buffer mode of the ICM loop (kcs_icm_run_host): y and x arrive from / x returns to HOST memory in z chunks.
-#define KCS_MAX_CHUNKS 9
-struct HostIO {
-    const float *hy;   // [host] y[T][nz][A][B]
-    float *hx;         // [host] x[T][nz][ny][nx], in and out
-    int nchunk;
-    int zb[KCS_MAX_CHUNKS + 1];  // chunk k = slices [zb[k], zb[k + 1])
-    cudaEvent_t ev_lam;          // lambda (copied in last: only MAP-LM reads it) is on the device
-};
-
 // The z chunks of the host-buffer pipeline.  Nothing can run before the first chunk has arrived, and the last chunk's x
 // leaves behind MAP-LM anyway: the LEAD chunk is the smallest that fills the GPU once (148 SMs x 6 forward CTAs of 128
 // ray lanes), each following chunk is twice the one before (the OS pass of a slice takes about twice its copy), up to a
@@ -636,7 +654,7 @@ static void plan_chunks(const kcs_ctx *c, HostIO &io) {
 // right after its last OSL update of the last iteration.
 static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, float scale, float *x, float *theta,
                         float *lambda, float beta_first, float beta, float gamma, float delta, int n_lm, int n_iter,
-                        const HostIO *io) {
+                        HostIO *io) {
     if (!c) return KCS_ERR_NULL;
     if (!y || !r || !x || !theta || !lambda) return fail(c, KCS_ERR_NULL, "kcs_icm: NULL buffer");
     if (r_mode != KCS_R_PER_FRAME && r_mode != KCS_R_FULL) return fail(c, KCS_ERR_SHAPE, "kcs_icm: unknown r_mode");
@@ -664,7 +682,9 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
     } restore{c, c->stream};
     cudaStream_t lanes[2] = {c->stream, c->os_stream};
     int rc;
-    if (n_iter > 0 && (rc = start_kinetic(c, theta, Tp))) return rc;  // beside the packing and the first forward projection
+    // beside the packing and the first forward projection; host-buffer mode: theta arrives chunk by chunk, the first
+    // iteration's model curve is evaluated per chunk on the chunk's lane
+    if (n_iter > 0 && !io && (rc = start_kinetic(c, theta, Tp))) return rc;
     if ((rc = ensure_border(c, Tp))) return rc;
     if (r_mode == KCS_R_PER_FRAME) {
         KCS_CUDA_OK(c, cudaMemsetAsync(c->r_pad, 0, KCS_MAX_FRAMES * sizeof(float), c->stream));
@@ -696,15 +716,16 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
             if (nzc == 0) continue;
             const int lane = k % nlane;
             c->stream = lanes[lane];
-            if (io && it == 0) {  // this chunk's x and y have been copied to the staging buffers: pack them
+            if (io && it == 0) {  // this chunk's x, y and theta have been copied to the staging buffers
                 KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_in[k], 0));
                 if ((rc = pack_image(c, x, T, c->xi, Tp, z0, nzc))) return rc;
                 if ((rc = pack_sino(c, y, T, c->yi, Tp, g.A, z0, nzc))) return rc;
+                if ((rc = kcs_launch_kinetic(c, theta, c->Fi, nullptr, 1, Tp, z0, nzc))) return rc;
             }
             for (int s = 0; s < g.S; ++s) {  // Q5: subsets in order 0..S-1
                 // after the first OSL update of this call x is zero outside the mask: rays are clipped to the FOV circle
                 if ((rc = kcs_launch_forward(c, Tp, s, 1, scale, r_mode, (it > 0 || s > 0) ? 1 : 0, z0, nzc))) return rc;
-                if (!has_F[lane]) {  // the model curve (second stream) is needed from the first OSL update on
+                if (!has_F[lane] && !(io && it == 0)) {  // the model curve (second stream) is needed from the first OSL update on
                     KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
                     has_F[lane] = true;
                 }
@@ -731,7 +752,7 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
             KCS_CUDA_OK(c, cudaEventRecord(c->ev_join, c->aux_stream));
         }
         if (io && it == 0) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, io->ev_lam, 0));
-        if ((rc = lm_steps(c, c->xi, 1, Tp, theta, lambda, gamma, delta, n_lm, nullptr))) return rc;
+        if ((rc = lm_steps(c, c->xi, 1, Tp, theta, lambda, gamma, delta, n_lm, nullptr, last ? io : nullptr))) return rc;
         if (last && !io) KCS_CUDA_OK(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
     }
     if (n_iter == 0) {
@@ -862,6 +883,12 @@ int kcs_icm_run_host(kcs_ctx *c, const float *y, const float *r, int r_mode, flo
         KCS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_lam, cudaEventDisableTiming));
     }
     io.ev_lam = c->ev_lam;
+    while ((int)c->ev_lm.size() < KCS_LM_PIECES) {
+        cudaEvent_t a = nullptr;
+        KCS_CUDA_OK(c, cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+        c->ev_lm.push_back(a);
+    }
+    for (int p = 0; p < KCS_LM_PIECES; ++p) io.ev_lm[p] = c->ev_lm[p];
     while ((int)c->ev_in.size() < io.nchunk) {
         cudaEvent_t a = nullptr, b = nullptr;
         KCS_CUDA_OK(c, cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
@@ -874,14 +901,15 @@ int kcs_icm_run_host(kcs_ctx *c, const float *y, const float *r, int r_mode, flo
     // may still be in use by a previous call)
     KCS_CUDA_OK(c, cudaEventRecord(c->ev_small, st));
     KCS_CUDA_OK(c, cudaStreamWaitEvent(in, c->ev_small, 0));
-    // order on the copy-in stream: theta and r (the model curve and the first ratio need them), the chunks, lambda last
-    KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_theta, theta, 4 * c->n_vox * sizeof(float), cudaMemcpyHostToDevice, in));
+    // order on the copy-in stream: r (the first ratio needs it), the chunks, lambda last (only MAP-LM reads it)
     KCS_CUDA_OK(c, cudaMemcpyAsync(c->st_r, r, nr * sizeof(float), cudaMemcpyHostToDevice, in));
     KCS_CUDA_OK(c, cudaEventRecord(c->ev_small, in));
-    for (int k = 0; k < io.nchunk; ++k) {  // x and y of chunk k: T strided pieces each (one 2-D copy)
+    for (int k = 0; k < io.nchunk; ++k) {  // x, y and theta of chunk k: T resp. 4 strided pieces each (one 2-D copy)
         const int z0 = io.zb[k], nzc = io.zb[k + 1] - io.zb[k];
         if (nzc > 0) {
             const size_t v2 = (size_t)g.ny * g.nx, r2 = (size_t)g.A * g.B;
+            KCS_CUDA_OK(c, cudaMemcpy2DAsync(c->st_theta + z0 * v2, c->n_vox * sizeof(float), theta + z0 * v2, c->n_vox * sizeof(float),
+                                             nzc * v2 * sizeof(float), 4, cudaMemcpyHostToDevice, in));
             KCS_CUDA_OK(c, cudaMemcpy2DAsync(c->st_x + z0 * v2, c->n_vox * sizeof(float), x + z0 * v2, c->n_vox * sizeof(float),
                                              nzc * v2 * sizeof(float), T, cudaMemcpyHostToDevice, in));
             KCS_CUDA_OK(c, cudaMemcpy2DAsync(c->st_y + z0 * r2, c->n_ray_all * sizeof(float), y + z0 * r2,
@@ -911,8 +939,19 @@ int kcs_icm_run_host(kcs_ctx *c, const float *y, const float *r, int r_mode, flo
     } else {
         KCS_CUDA_OK(c, cudaMemcpyAsync(x, c->st_x, nx_ * sizeof(float), cudaMemcpyDeviceToHost, st));
     }
-    KCS_CUDA_OK(c, cudaMemcpyAsync(theta, c->st_theta, 4 * c->n_vox * sizeof(float), cudaMemcpyDeviceToHost, st));
-    KCS_CUDA_OK(c, cudaMemcpyAsync(lambda, c->st_lambda, c->n_vox * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (io.n_piece > 0) {  // theta and lambda of a z piece leave while the last MAP-LM step fits the next piece
+        const size_t v2 = (size_t)g.ny * g.nx;
+        for (int p = 0; p < io.n_piece; ++p) {
+            const size_t z0 = (size_t)io.pzb[p], nzp = (size_t)(io.pzb[p + 1] - io.pzb[p]);
+            KCS_CUDA_OK(c, cudaStreamWaitEvent(out, io.ev_lm[p], 0));
+            KCS_CUDA_OK(c, cudaMemcpy2DAsync(theta + z0 * v2, c->n_vox * sizeof(float), c->st_theta + z0 * v2, c->n_vox * sizeof(float),
+                                             nzp * v2 * sizeof(float), 4, cudaMemcpyDeviceToHost, out));
+            KCS_CUDA_OK(c, cudaMemcpyAsync(lambda + z0 * v2, c->st_lambda + z0 * v2, nzp * v2 * sizeof(float), cudaMemcpyDeviceToHost, out));
+        }
+    } else {
+        KCS_CUDA_OK(c, cudaMemcpyAsync(theta, c->st_theta, 4 * c->n_vox * sizeof(float), cudaMemcpyDeviceToHost, st));
+        KCS_CUDA_OK(c, cudaMemcpyAsync(lambda, c->st_lambda, c->n_vox * sizeof(float), cudaMemcpyDeviceToHost, st));
+    }
     KCS_CUDA_OK(c, cudaStreamSynchronize(st));
     KCS_CUDA_OK(c, cudaStreamSynchronize(out));
     KCS_CUDA_OK(c, cudaStreamSynchronize(in));

@@ -141,6 +141,7 @@ struct kcs_ctx {
     cudaStream_t in_stream, out_stream;
     cudaEvent_t ev_small, ev_lam;          // theta and r / lambda are on the device
     std::vector<cudaEvent_t> ev_in, ev_out;  // per chunk: inputs have arrived / x is final on the device
+    std::vector<cudaEvent_t> ev_lm;          // per z piece of the last MAP-LM step: theta, lambda are final on the device
 };
 
 #define KCS_CUDA_OK(ctx, call)                                                                  \
@@ -207,9 +208,11 @@ int kcs_launch_osl_planar(kcs_ctx *c, float *x, const float *bp, const float *se
 
 // ---- launchers (kcs_kinetic.cu) ------------------------------------------------------------------
 // F (and J) from theta.  inner == 0: F planar [T][V], J planar [4][T][V] or NULL;  inner == 1: F = padded inner layout, Tp.
-int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp);
+// (z0, nzc): slices [z0, z0 + nzc) only (inner == 1, J == NULL); nzc < 0 = up to the last slice.
+int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp, int z0 = 0, int nzc = -1);
 int kcs_launch_ki_map(kcs_ctx *c, const float *theta, float *ki);
 // one Jacobi LM step: reads theta_in, writes theta_out for the in-mask voxels (masked-out voxels are never touched).
 //   x_inner == 0: x planar [T][V];  x_inner == 1: x = c->xi padded inner layout with Tp.
 int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const void *theta_in, int in_f64, void *theta_out,
-                       int out_f64, const void *lam_in, void *lam_out, float gamma, float delta, float *cost);
+                       int out_f64, const void *lam_in, void *lam_out, float gamma, float delta, float *cost, int z0 = 0,
+                       int nzc = -1);  // slices [z0, z0 + nzc) only (Jacobi: a step reads theta_in, so z ranges are independent)

@@ -222,12 +222,12 @@ __global__ void __launch_bounds__(128) k_kinetic(KGeom g, KKin kin, const float 
 // zeros it was created with), written to the padded frame-innermost layout four frames at a time (one 16 B store per
 // lane instead of four scattered 4 B stores; frames T..Tp-1 are written as 0).
 __global__ void __launch_bounds__(128) k_kinetic_inner(KGeom g, KKin kin, const float *__restrict__ theta, float *F, long long nvox,
-                                                       const int *__restrict__ vlist, int M2, int Tp) {
+                                                       const int *__restrict__ vlist, int M2, int Tp, long long t0, long long t1) {
     extern __shared__ double sh_raw[];
     KFrame *fr = reinterpret_cast<KFrame *>(sh_raw);
     load_frames(kin, fr);
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= (long long)M2 * g.nz) return;
+    const long long t = t0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;  // [t0, t1): the in-mask voxels of a z range
+    if (t >= t1) return;
     const int v2 = g.nx * g.ny;
     const int z = (int)(t / M2), rem = vlist[(int)(t - (long long)z * M2)];
     const long long v = (long long)z * v2 + rem;
@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
                                                  const TI *lam_in, TO *lam_out,  // may alias: each thread touches its own element
                                                  const unsigned char *__restrict__ mask, const int *__restrict__ vlist, int M2,
                                                  long long nvox, double gamma, LmOpt o, float *cost,
-                                                 double *__restrict__ st, long long nfit) {
+                                                 double *__restrict__ st, long long nfit, long long t0, long long t1) {
     constexpr int NQ = OPT ? 10 : 6;
     constexpr bool WLS = OPT;
     // FIRST step of a call (fp32 input): the data part of the normal equations is evaluated at theta.  Later steps read
@@ -335,8 +335,8 @@ __global__ void __launch_bounds__(KCS_LM_TPB, KCS_LM_MINBLK) k_lm_step(KGeom g, 
     extern __shared__ double sh_raw[];
     KFrame *fr = reinterpret_cast<KFrame *>(sh_raw);
     load_frames(kin, fr);
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= (long long)M2 * g.nz) return;
+    const long long t = t0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;  // [t0, t1): the in-mask voxels of a z range
+    if (t >= t1) return;
     const int v2 = g.nx * g.ny;
     const int z = (int)(t / M2), rem = vlist[(int)(t - (long long)z * M2)];
     const long long v = (long long)z * v2 + rem;
@@ -455,14 +455,16 @@ int kcs_launch_ki_map(kcs_ctx *c, const float *theta, float *ki) {
     return KCS_OK;
 }
 
-int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp) {
+int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int inner, int Tp, int z0, int nzc) {
     const long long nvox = (long long)c->n_vox;
     const size_t smem = sizeof(KFrame) * c->kin.T;
+    if (nzc < 0) nzc = c->g.nz - z0;
     ProfScope ps(c, KCS_K_KINETIC);
     if (inner && !J) {
-        const long long nfit = (long long)c->n_inmask2 * c->g.nz;
+        const long long t0 = (long long)c->n_inmask2 * z0, nfit = (long long)c->n_inmask2 * nzc;
         if (nfit > 0)
-            k_kinetic_inner<<<(unsigned)((nfit + 127) / 128), 128, smem, c->stream>>>(c->g, c->kin, theta, F, nvox, c->d_vlist, c->n_inmask2, Tp);
+            k_kinetic_inner<<<(unsigned)((nfit + 127) / 128), 128, smem, c->stream>>>(c->g, c->kin, theta, F, nvox, c->d_vlist, c->n_inmask2, Tp,
+                                                                                      t0, t0 + nfit);
     } else
         k_kinetic<<<(unsigned)((nvox + 127) / 128), 128, smem, c->stream>>>(c->g, c->kin, theta, F, J, nvox, inner, Tp);
     LAUNCH_CHECK(c);
@@ -471,12 +473,14 @@ int kcs_launch_kinetic(kcs_ctx *c, const float *theta, float *F, float *J, int i
 
 // in_f64 / out_f64: 0 = fp32 buffers (the caller's), 1 = the context's fp64 ping-pong buffers.
 int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const void *theta_in, int in_f64, void *theta_out,
-                       int out_f64, const void *lam_in, void *lam_out, float gamma, float delta, float *cost) {
+                       int out_f64, const void *lam_in, void *lam_out, float gamma, float delta, float *cost, int z0, int nzc) {
     const long long nvox = (long long)c->n_vox;
     const size_t smem = sizeof(KFrame) * c->kin.T;
-    const long long nfit = (long long)c->n_inmask2 * c->g.nz;
-    if (nfit == 0) return KCS_OK;
-    const unsigned grid = (unsigned)((nfit + KCS_LM_TPB - 1) / KCS_LM_TPB);
+    const long long nfit = (long long)c->n_inmask2 * c->g.nz;  // stride of the carried sums: always the whole volume
+    if (nzc < 0) nzc = c->g.nz - z0;
+    const long long t0 = (long long)c->n_inmask2 * z0, t1 = t0 + (long long)c->n_inmask2 * nzc;
+    if (t1 == t0) return KCS_OK;
+    const unsigned grid = (unsigned)((t1 - t0 + KCS_LM_TPB - 1) / KCS_LM_TPB);
     ProfScope ps(c, KCS_K_LM);
     LmOpt o;
     o.fixmask = 0;
@@ -492,7 +496,7 @@ int kcs_launch_lm_step(kcs_ctx *c, const float *x, int x_inner, int Tp, const vo
 #define KCS_LM_GO2(TI, TO, OPT)                                                                                        \
     k_lm_step<TI, TO, OPT><<<grid, KCS_LM_TPB, smem, c->stream>>>(c->g, c->kin, x, x_inner, Tp, (const TI *)theta_in, (TO *)theta_out, \
                                                        (const TI *)lam_in, (TO *)lam_out, c->d_mask, c->d_vlist, c->n_inmask2, nvox, (double)gamma,  \
-                                                       o, cost, c->lm_state, nfit)
+                                                       o, cost, c->lm_state, nfit, t0, t1)
 #define KCS_LM_GO(TI, TO) do { if (opt) KCS_LM_GO2(TI, TO, true); else KCS_LM_GO2(TI, TO, false); } while (0)
     if (!in_f64 && !out_f64) KCS_LM_GO(float, float);
     else if (!in_f64 && out_f64) KCS_LM_GO(float, double);
