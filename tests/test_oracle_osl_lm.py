@@ -259,3 +259,34 @@ def test_icm_runs_and_improves(tiny):
         err.append(np.linalg.norm(x - p["x_true"]) / np.linalg.norm(p["x_true"]))
     assert ll[-1] > ll[0] and err[-1] < err[0]
     assert np.all(th[:, :, mask == 0] == 0) and np.all(x[:, :, mask == 0] == 0)
+
+
+def test_icm_joint_fixed_point_and_contraction(tiny):
+    """I on CONSISTENT data, y = scale A x* + r with x* = K(theta*): the pair (x*, theta*) is a fixed point of
+    the whole iteration with the kinetic prior on -- the ratio is 1, the prior term vanishes at x = F, the fit's gradient
+    vanishes at x = K(theta) -- and from a perturbed theta the iteration moves back towards it.  With uniform maps the
+    Huber gradient vanishes too (in-mask neighbours only), so the fixed point survives gamma > 0."""
+    cfg, o, mask, p = tiny
+    m = mask > 0
+    lam0 = np.zeros((cfg["nz"], cfg["ny"], cfg["nx"]))
+    th, xs = p["theta_true"], p["x_true"]
+    x1, th1, _ = o.icm_iteration(p["ybar"], p["r"], p["scale"], xs, th, lam0, 0.1, 0.0, 0.01, 3)
+    assert np.abs(x1 - xs).max() <= 1e-10 * xs.max()
+    assert np.abs(th1 - th).max() <= 1e-8
+    # perturbed maps, exact activity: one iteration (5 LM steps) removes most of the perturbation, the prior's pull on x
+    # (towards the curve of the perturbed maps) stays a fraction of the distance between the two curves
+    th_p = th * (1.0 + 0.1 * (ki.uniform(th.shape, seed=5) - 0.5))
+    F_p = o.kinetic_eval(th_p) * mask[None, None]
+    x2, th2, _ = o.icm_iteration(p["ybar"], p["r"], p["scale"], xs, th_p, lam0, 0.1, 0.0, 0.01, 5)
+    e0 = np.linalg.norm((th_p - th)[:, :, m])
+    e2 = np.linalg.norm((th2 - th)[:, :, m])
+    assert e2 < 0.5 * e0, (e0, e2)
+    assert np.linalg.norm(x2 - xs) < 0.5 * np.linalg.norm(F_p - xs)
+    assert np.linalg.norm(x2 - xs) > 0  # beta = 0.1 did act
+    # uniform maps, Huber prior on
+    th_u = np.array(ki.THETA0)[:, None, None, None] * mask[None, None].astype(np.float64)
+    x_u = o.kinetic_eval(th_u) * mask[None, None]
+    y_u = p["scale"] * o.forward_project(x_u, -1) + p["r"][:, None, None, None]
+    x3, th3, _ = o.icm_iteration(y_u, p["r"], p["scale"], x_u, th_u, lam0, 0.1, 1e4, 0.01, 3)
+    assert np.abs(x3 - x_u).max() <= 1e-10 * x_u.max()
+    assert np.abs(th3 - th_u)[:, :, m].max() <= 1e-8
