@@ -83,6 +83,10 @@ def test_static_forward_projection_matches_the_context_path():
             for g, w in zip(got, want):
                 assert bool(torch.isfinite(g).all())
                 assert close(g, w[:nf]), (cfg["name"] if "name" in cfg else (nx, ny, nz), subset, nf)
+            if nx == 61 and nf == T:          # and against the oracle itself, on the geometry it finishes in a moment
+                from oracle import Oracle
+                yo = Oracle(cfg).forward_project(xs[0].cpu().numpy().astype(np.float64), subset)
+                assert close(got[0], torch.tensor(yo, device="cuda")), ("oracle", subset)
             if calls > 2 and nf == T:         # past the first call (module load): the device's free memory does not move
                 assert abs(free0 - free1) < (2 << 20), (free0, free1)
         ctx.close()
