@@ -17,7 +17,7 @@ single-GPU configuration (BASELINE's `metric` names no config).
   e2e        the same metric through kcs_icm_run_host with pinned HOST buffers: H2D of y, r, x, theta, lambda and D2H
              of x, theta, lambda inside the timed region of every step.
   roofline   the dominant kernel class of the step (per-kernel CUDA events from kcs_profile_*, a second pass of the
-             same K steps).  SURVEY.md 8(d): T_lb = max(HBM bytes / BW_HBM, L2 bytes / BW_L2, flops / P_FP32); `bound`
+             same K steps, every kernel launched over the whole volume on one stream).  SURVEY.md 8(d): T_lb = max(HBM bytes / BW_HBM, L2 bytes / BW_L2, flops / P_FP32); `bound`
              names the largest term, frac = T_lb / measured launch time; achieved / peak are that term's.  All three
              terms, for every kernel class, are under `roofline.classes`.  BW_HBM = MEASURED_PEAKS.json; BW_L2 and
              P_FP32 / P_FP64 are measured in this run by libkcs_probe.so (include/kcs_probe.h).  Units are the EXECUTED
@@ -467,6 +467,9 @@ def run_ours(args):
             "step_t_lb_ms": sum(classes[k]["t_lb_ms"] * per_class[k]["launches_per_step"] for k in classes),
             "step_frac": sum(classes[k]["t_lb_ms"] * per_class[k]["launches_per_step"] for k in classes) / ms_per_step,
             "classes": classes,
+            # kcs_icm_run splits the OS pass of a large volume in two z halves on two streams; with per-kernel timing on it
+            # launches every kernel over the whole volume on one stream, so that the events bracket kernels running alone
+            "profile_pass": "one stream, full-volume launches (timed steps: two z halves on two streams)",
         }
 
     # ---- end to end through the host-buffer entry point

@@ -661,14 +661,17 @@ static int icm_run_impl(kcs_ctx *c, const float *y, const float *r, int r_mode, 
     if (n_lm < 0 || n_iter < 0 || !(scale > 0.f)) return fail(c, KCS_ERR_SHAPE, "kcs_icm: bad n_lm / n_iter / scale");
     const KGeom &g = c->g;
     const int T = c->cfg.n_frames, Tp = round_up4(T);
-    // Host-buffer mode: two LANES (the context's stream and a second one) carry the OS pass of alternate z chunks.  Direct
-    // planes are independent, and while one chunk's kernel drains its last CTAs the other chunk's kernel fills the SMs: a
-    // chunk launch ends in a tail of ~0.1 ms, 42 times per chunk and iteration.  (A device-resident call is one chunk on
-    // the context's stream: split in two halves the C4 iteration gains 1 %, and per-kernel timing wants kernels that have
-    // the GPU to themselves.)
-    const bool two = io != nullptr && io->nchunk >= 2 && !c->prof_on;
-    const int whole[2] = {0, g.nz};
-    const int nchunk = io ? io->nchunk : 1;
+    // Two LANES (the context's stream and a second one) carry the OS pass of alternate z chunks.  Direct planes are
+    // independent, and while one chunk's kernel drains its last CTAs the other chunk's kernel fills the SMs (every launch
+    // ends in a tail of ~0.1 ms, 42 times per chunk and iteration).  Host-buffer mode: the chunks of the copy pipeline.
+    // Device-resident call: the volume in two halves -- C2 0.85 -> 0.74 ms (inside its CUDA graph), C3 8.17 -> 7.48 ms,
+    // C4 131.8 -> 130.6 ms per iteration; more chunks do not pay (C3: 3 / 4 / 6 / 8 chunks 7.99 / 7.43 / 7.48 / 8.11 ms).
+    // One lane for volumes too small to split and while per-kernel timing is on: its events must bracket kernels that
+    // have the GPU to themselves.  The result does not depend on the split, bit for bit.
+    const bool res2 = !io && !c->prof_on && (double)c->n_vox * T >= 1.0e6 && g.nz >= 8;
+    const bool two = (io != nullptr && io->nchunk >= 2 && !c->prof_on) || res2;
+    const int whole[3] = {0, res2 ? g.nz / 2 : g.nz, g.nz};
+    const int nchunk = io ? io->nchunk : (res2 ? 2 : 1);
     const int *zb = io ? io->zb : whole;
     const int nlane = two ? 2 : 1;
     if (two && !c->os_stream) {

@@ -139,7 +139,7 @@ struct kcs_ctx {
     // kcs_icm_run_host: the volume moves in z chunks; chunk k + 1 is copied in (in_stream) and chunk k - 1 copied out
     // (out_stream) while chunk k goes through its OS pass on the context's stream
     cudaStream_t in_stream, out_stream;
-    cudaEvent_t ev_small, ev_lam;          // theta and r / lambda are on the device
+    cudaEvent_t ev_small, ev_lam;          // r / lambda are on the device (theta arrives with the chunks)
     std::vector<cudaEvent_t> ev_in, ev_out;  // per chunk: inputs have arrived / x is final on the device
     std::vector<cudaEvent_t> ev_lm;          // per z piece of the last MAP-LM step: theta, lambda are final on the device
 };
