@@ -10,7 +10,9 @@ arithmetic is not involved in the comparison (both chains are the oracle): the l
 fit), i.e. the floor under which no fp32 OS pass can stay.  Measured with KCS_FLOOR_FULL=1 (C2 at full size, 8 slices):
 min over the parameters 99.82 % after 10 iterations (profiles/r2_oracle_noise_floor_C2.txt); the CUDA path reaches
 99.85-99.88 % on the same data.  KCS_FLOOR_FULL=C3 (C3 at full size, 2 counts per voxel-frame): 98.93 %, activity 1.26e-3
-(profiles/r2_oracle_noise_floor_C3.txt); the CUDA path: 98.8 %, 1.30e-3.  The default run uses 2 slices of C2 so that the CPU suite stays short.
+(profiles/r2_oracle_noise_floor_C3.txt); the CUDA path: 98.8 %, 1.30e-3.  KCS_FLOOR_FULL=C4z4 (C4's in-plane geometry on 4
+slices, the third chain of tests/test_gpu_fullsize.py): 98.98 %, 1.79e-3 (profiles/r2_oracle_noise_floor_C4z4.txt); the CUDA
+path: 98.7 %, 2.2e-3.  The default run uses 2 slices of C2 so that the CPU suite stays short.
 
     KCS_FLOOR_FULL=1 python -m pytest tests/test_oracle_noise_floor.py -s -q
 """
@@ -50,9 +52,12 @@ def chain_pair(cfg, rms, seed=99):
 
 def test_fp32_sized_perturbation_is_amplified_past_the_tolerance_band():
     env = os.environ.get("KCS_FLOOR_FULL", "")
-    full = env in ("1", "C2", "C3")
-    name = "C3" if env == "C3" else "C2"             # KCS_FLOOR_FULL=C3: the same experiment on C3 at full size (~10 min)
-    cfg = ki.config(name)
+    full = env in ("1", "C2", "C3", "C4z4")
+    name = env if env in ("C3", "C4z4") else "C2"    # KCS_FLOOR_FULL=C3: the same experiment on C3 at full size (~10 min)
+    if name == "C4z4":                               # C4's in-plane geometry on 4 slices, the chain of tests/test_gpu_fullsize.py
+        cfg = (lambda c: dict(c, nz=4, counts=c["counts"] * 4 / c["nz"]))(ki.config("C4"))
+    else:
+        cfg = ki.config(name)
     if not full:
         cfg = dict(cfg, nz=2, counts=cfg["counts"] * 2 / cfg["nz"])
     rows = chain_pair(cfg, RMS)
